@@ -1,0 +1,141 @@
+/* lx.h — C ABI of liblx: B200-native (sm_100a) 3-centre Coulomb integrals (X|ab) and integral-direct DF-J.
+ *
+ * Everything the hot path computes is defined by arxiv 2210.03192 (cited below as PAPER.md:<line>):
+ *   (X_c|a b) = Σ_k Σ_i Σ_j c_k c_i c_j [c|ab]_{kij}                          contracted shell-set
+ *   [c|ab]    = ∬ φ_c(r1) |r1−r2|⁻¹ φ_a(r2) φ_b(r2) dr1 dr2                   eq. 12, Coulomb :455
+ *   φ_a(r)    = (x−A_x)^{a_x}(y−A_y)^{a_y}(z−A_z)^{a_z} exp(−ζ_a|r−A|²)      eq. 13, unnormalised
+ * evaluated by the Obara–Saika/HGPA scheme of PAPER.md §2.5 (lines 104–124): Boys → [00|0]^(m) (eq. 4) → VRR1
+ * (eq. 3) → VRR2 → contraction → HRR (eq. 1), and fused with the density-fitting contractions
+ *   γ_X  = Σ_ab (X|ab) D_ab ,   J_ab = Σ_X (X|ab) d_X
+ * through a "digestion" step that replaces the store, so the 3-centre tensor is never written.
+ *
+ * Conventions common to every entry point
+ *   - Pointers are DEVICE pointers unless the name ends in _host.  The caller owns every buffer; the library never
+ *     frees or keeps caller memory.  The only library-owned device memory is the Boys table made by lx_init().
+ *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream) and return
+ *     before completion.  lx_shells_t structs themselves live on the HOST; their array members are device pointers
+ *     (host pointers for the *_host arguments of lx_schedule_create).
+ *   - Return value: LX_OK (0) or a negative LX_E* code.  Nothing throws, prints or exits.
+ *   - Cartesian component order inside a shell of angular momentum l (reading G2 of DESIGN.md):
+ *       for lx = l..0, for ly = l−lx..0, lz = l−lx−ly          (xx, xy, xz, yy, yz, zz for l = 2)
+ *     nc(l) = (l+1)(l+2)/2.  The aux index X is Cartesian as well (reading G1).
+ *   - `coef` already contains every normalisation factor; the library multiplies by coef only (reading G3,
+ *     PAPER.md:439, 453).  Units: bohr / Hartree.
+ *   - Compiled class range: 0 ≤ lx ≤ LX_MAX_L_AUX, 0 ≤ la, lb ≤ LX_MAX_L_PRIM; anything else → LX_EUNSUPPORTED.
+ */
+#ifndef LX_H
+#define LX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LX_MAX_L_AUX 6
+#define LX_MAX_L_PRIM 4
+
+#define LX_OK 0
+#define LX_EINVAL (-1)        /* null / negative / inconsistent argument                                       */
+#define LX_EUNSUPPORTED (-2)  /* class outside the compiled range                                               */
+#define LX_ENOMEM (-3)        /* workspace too small (see the *_workspace_bytes functions)                      */
+#define LX_ECUDA (-4)         /* CUDA runtime error; text via lx_strerror(LX_ECUDA)                             */
+#define LX_ENOTINIT (-5)      /* lx_init() has not been called on this device                                   */
+
+/* Gaussian shell table, structure of arrays (a shell is a centre, exponents ζ, contraction
+ * coefficients and l, over unnormalised primitives).  Immutable during a call. */
+typedef struct {
+    int32_t nshell;
+    const int32_t *L;        /* [nshell]    angular momentum l                                                  */
+    const int32_t *K;        /* [nshell]    contraction degree (= prim_off[i+1]-prim_off[i])                    */
+    const int32_t *prim_off; /* [nshell+1]  offsets into zeta / coef                                            */
+    const double *center;    /* [nshell*3]  x,y,z in bohr                                                       */
+    const double *zeta;      /* [nprim]     exponents ζ                                                         */
+    const double *coef;      /* [nprim]     coefficients including normalisation                                */
+    const int32_t *bf_off;   /* [nshell+1]  first Cartesian basis-function index (DF calls only; may be NULL
+                                            for lx_eri3_batch)                                                  */
+} lx_shells_t;
+
+/* Library state.  lx_init builds the Boys-function interpolation table (PAPER.md:132 and eq. 19:
+ * F_m(x) = ∫_0^1 y^{2m} exp(−x y²) dy) on the host in long double and uploads it to `device`; it also raises the
+ * dynamic shared-memory limit of every kernel.  Idempotent.  lx_finalize frees the table. */
+int lx_init(int device);
+int lx_finalize(void);
+const char *lx_strerror(int status);
+/* Version / build string of the library ("lx3 <n> sm_100a ..."), static storage. */
+const char *lx_version(void);
+
+/* lx_eri3_batch — PAPER.md §2.5 (lines 104–124), SURVEY.md §8(a) rows a1–a8.
+ * Computes the full shell-sets (X|ab) for every listed primary shell pair × every listed aux shell of ONE class:
+ *   out[((p*nx + x)*nc(lx) + cx)*nc(la)*nc(lb) + ca*nc(lb) + cb] = (X_cx | a_ca b_cb),
+ *   a = pair_idx[2p], b = pair_idx[2p+1], X = x_idx[x];  dense, row-major, fully overwritten.
+ * All aux shells listed must have L = lx and all pairs L = (la, lb): the caller's contract (not checked on the
+ * device).  la < lb is legal: the library swaps the roles of the two shells internally and still writes [ca][cb] in
+ * the caller's order.  No screening is applied (reading G13).  Degenerate geometry (A = B, P = C, all centres
+ * equal, the same shell twice in a pair) is legal (reading G15).
+ *   x_idx [nx], pair_idx [npair*2]: device int32.   out: device double, npair*nx*nc(lx)*nc(la)*nc(lb) elements.
+ *   workspace: device scratch of at least lx_eri3_workspace_bytes(...) bytes (primitive-pair data, row a1).
+ * nx == 0 or npair == 0 is a no-op returning LX_OK.
+ * Errors: LX_EINVAL (null pointer with non-zero count, negative count), LX_EUNSUPPORTED, LX_ENOMEM, LX_ENOTINIT,
+ * LX_ECUDA. */
+int lx_eri3_batch(int lx, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim,
+                  const int32_t *x_idx, int nx, const int32_t *pair_idx, int npair, double *out,
+                  void *workspace, size_t workspace_bytes, void *stream);
+
+/* Workspace size for lx_eri3_batch: kmax_pair = max over listed pairs of K_a*K_b (contraction degrees). */
+size_t lx_eri3_workspace_bytes(int lx, int la, int lb, int nx, int npair, int kmax_pair);
+
+/* Schedule — SURVEY.md §8(a) row a0; PAPER.md:54 (batches per class), :365 ("identical screening").
+ * Built once per basis on the HOST from host copies of the shell tables.  Buckets aux shells by L and shell pairs
+ * by (La, Lb) (pairs with La < Lb are stored swapped), orders every bucket by contraction degree and then by
+ * Schwarz factor descending, so that for every pair the aux shells that survive
+ *        q_aux[X] * q_pair[p] >= tau          (evaluated in double; a set with the product < tau is skipped)
+ * form a prefix of the aux bucket; stores the prefix length per (pair, lx).  q_aux_host [aux.nshell] and q_pair_host
+ * [npair] are Schwarz factors Q_X = sqrt(max (X|X)), Q_ab = sqrt(max (ab|ab)) supplied by the caller; if either is
+ * NULL no screening is applied.  pair_idx_host [npair*2] lists the unique shell pairs (a,b) to visit; a pair with
+ * a == b is weighted once, a != b stands for both (a,b) and (b,a) (reading G16).
+ * The schedule owns small device copies of its index lists (freed by lx_schedule_destroy). */
+typedef struct lx_schedule lx_schedule_t;
+int lx_schedule_create(const lx_shells_t *aux_host, const lx_shells_t *prim_host, const double *q_aux_host,
+                       const double *q_pair_host, const int32_t *pair_idx_host, int npair, double tau,
+                       lx_schedule_t **out);
+int lx_schedule_destroy(lx_schedule_t *s);
+/* Number of unscreened shell-sets / Cartesian integrals one DF pass evaluates (reading G19). */
+int64_t lx_schedule_num_sets(const lx_schedule_t *s);
+int64_t lx_schedule_num_integrals(const lx_schedule_t *s);
+/* Workspace (bytes) needed by lx_df_gamma / lx_df_J with this schedule. */
+size_t lx_df_workspace_bytes(const lx_schedule_t *s);
+
+/* lx_df_gamma — SURVEY.md §8(a) row a9 (PAPER.md:283 digestion callable, :365).
+ *   gamma[bf(X)+cx] = Σ_{pairs p=(a,b)} f_p Σ_{ca,cb} (X_cx|a_ca b_cb) D[(bf(a)+ca)*ldD + bf(b)+cb],
+ *   f_p = 2 if a != b else 1, over the unscreened sets of the schedule.  D (nbf×nbf, leading dimension ldD) is read
+ *   as symmetric.  gamma [naux_bf] is overwritten.  FP64 atomics are used across thread blocks, so the last bits
+ *   may differ from run to run (reading G14).
+ * lx_df_J — row a10.
+ *   J[(bf(a)+ca)*ldJ + bf(b)+cb] = Σ_{X,cx} (X_cx|a_ca b_cb) d[bf(X)+cx], mirrored to (b,a); J (nbf×nbf) is
+ *   overwritten in full (blocks of unlisted or fully screened pairs become zero).
+ * aux / prim: the same tables the schedule was built from, with DEVICE array members (bf_off required). */
+int lx_df_gamma(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *D, int ldD,
+                double *gamma, void *workspace, size_t workspace_bytes, void *stream);
+int lx_df_J(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *d, double *J,
+            int ldJ, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Host-buffer convenience path (used for the end-to-end measurement): same result as lx_eri3_batch but every
+ * array member of aux/prim, x_idx, pair_idx and out are HOST pointers; the call allocates device scratch, copies
+ * in, runs, copies out and synchronises.  Returns after `out_host` is complete. */
+int lx_eri3_batch_host(int lx, int la, int lb, const lx_shells_t *aux_host, const lx_shells_t *prim_host,
+                       const int32_t *x_idx_host, int nx, const int32_t *pair_idx_host, int npair,
+                       double *out_host);
+
+/* Boys function F_m(T), m = 0..mmax, for n values of T — the device routine the integral kernels use (row a2),
+ * exported for the accuracy sweep.  T [n] and out [n*(mmax+1)] are device pointers; mmax <= 18. */
+int lx_boys(const double *T, int n, int mmax, double *out, void *stream);
+
+/* Number of kernel launches the library has issued since lx_init (for the bench's `gpu_launches` claim). */
+int64_t lx_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LX_H */

@@ -1,0 +1,542 @@
+// lx_api.cu — C-ABI entry points of liblx (include/lx.h): library state, Boys table, primitive-pair pre-pass,
+// class dispatch, the Schwarz-screened schedule and the DF drivers.
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "lx_common.cuh"
+#include "lx_dispatch.h"
+
+namespace lx {
+
+// ------------------------------------------------------------------------------------------------ library state
+struct State {
+    bool ready = false;
+    int device = -1;
+    int num_sms = 0;
+    double *boys_tab = nullptr;      // [BOYS_NGRID][BOYS_MROWS]
+    std::atomic<long long> launches{0};
+    char cuda_msg[256] = "no CUDA error recorded";
+    // grow-only device arena for the host-buffer convenience path
+    void *arena = nullptr;
+    size_t arena_bytes = 0;
+    void *pinned = nullptr;
+    size_t pinned_bytes = 0;
+};
+static State g;
+static std::mutex g_mu;
+
+static int cuda_fail(cudaError_t e) {
+    snprintf(g.cuda_msg, sizeof(g.cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return LX_ECUDA;
+}
+#define LX_CUDA(expr)                                 \
+    do {                                              \
+        cudaError_t _e = (expr);                      \
+        if (_e != cudaSuccess) return cuda_fail(_e);  \
+    } while (0)
+
+static const launch_fn k_launch[3][7] = {
+    {launch_lx0_mode0, launch_lx1_mode0, launch_lx2_mode0, launch_lx3_mode0, launch_lx4_mode0, launch_lx5_mode0, launch_lx6_mode0},
+    {launch_lx0_mode1, launch_lx1_mode1, launch_lx2_mode1, launch_lx3_mode1, launch_lx4_mode1, launch_lx5_mode1, launch_lx6_mode1},
+    {launch_lx0_mode2, launch_lx1_mode2, launch_lx2_mode2, launch_lx3_mode2, launch_lx4_mode2, launch_lx5_mode2, launch_lx6_mode2},
+};
+
+// ------------------------------------------------------------------------------------------------ Boys table (host)
+// F_m(T) = ∫_0^1 y^{2m} exp(−T y²) dy (eq. 19) on the grid T_i = i/16 in long double:
+// positive-term series at the top order, then downward recursion.  Written for this library; shares nothing with
+// the test oracle.
+static void boys_table_host(std::vector<double> &tab) {
+    tab.assign((size_t)BOYS_NGRID * BOYS_MROWS, 0.0);
+    const int M = BOYS_MROWS - 1;
+    std::vector<long double> F(BOYS_MROWS);
+    for (int i = 0; i < BOYS_NGRID; ++i) {
+        const long double T = (long double)i / (long double)BOYS_PER_UNIT;
+        const long double eT = expl(-T);
+        long double term = 1.0L / (long double)(2 * M + 1), sum = term;
+        for (int n = 1; n < 4000; ++n) {
+            term *= (2.0L * T) / (long double)(2 * M + 2 * n + 1);
+            sum += term;
+            if (term < 1e-24L * sum) break;
+        }
+        F[M] = eT * sum;
+        for (int m = M; m >= 1; --m) F[m - 1] = (2.0L * T * F[m] + eT) / (long double)(2 * m - 1);
+        for (int m = 0; m < BOYS_MROWS; ++m) tab[(size_t)i * BOYS_MROWS + m] = (double)F[m];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ kernels
+// a1: primitive-pair data, one thread per (pair, primitive pair).  P by eq. 16, γ by eq. 14, K_ij = c_i c_j
+// exp(−ζaζb/γ |AB|²) (exponential factor of eq. 4).
+__global__ void pair_data_kernel(DevShells prim, const int32_t *__restrict__ pair_list, int npair, int swapped,
+                                 const long long *__restrict__ pd_off, int kstride, int kiter, double *__restrict__ pd) {
+    // flat index over pairs × kiter lanes; a lane walks ij = lane, lane+kiter, ... < K_a K_b
+    const long long total = (long long)npair * kiter;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long p = t / kiter;
+        const int lane = (int)(t - p * kiter);
+        const int a = pair_list[2 * p + swapped], b = pair_list[2 * p + 1 - swapped];
+        const int Ka = prim.K[a], Kb = prim.K[b];
+        const int Kab = min(Ka * Kb, kstride);
+        const double Ax = prim.center[3 * a], Ay = prim.center[3 * a + 1], Az = prim.center[3 * a + 2];
+        const double Bx = prim.center[3 * b], By = prim.center[3 * b + 1], Bz = prim.center[3 * b + 2];
+        const double r2 = (Ax - Bx) * (Ax - Bx) + (Ay - By) * (Ay - By) + (Az - Bz) * (Az - Bz);
+        for (int ij = lane; ij < Kab; ij += kiter) {
+            const int i = ij / Kb, j = ij - i * Kb;
+            const double za = prim.zeta[prim.prim_off[a] + i], zb = prim.zeta[prim.prim_off[b] + j];
+            const double ca = prim.coef[prim.prim_off[a] + i], cb = prim.coef[prim.prim_off[b] + j];
+            const double gam = za + zb, ig = 1.0 / gam;
+            const long long o = ((pd_off ? pd_off[p] : p * (long long)kstride) + ij) * 5;
+            pd[o + 0] = gam;
+            pd[o + 1] = (za * Ax + zb * Bx) * ig;
+            pd[o + 2] = (za * Ay + zb * By) * ig;
+            pd[o + 3] = (za * Az + zb * Bz) * ig;
+            pd[o + 4] = ca * cb * exp(-za * zb * ig * r2);
+        }
+    }
+}
+
+__global__ void boys_kernel(const double *__restrict__ tab, const double *__restrict__ T, int n, int mmax,
+                            double *__restrict__ out) {
+    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= (long long)n * (mmax + 1)) return;
+    const int i = (int)(t / (mmax + 1)), m = (int)(t - (long long)i * (mmax + 1));
+    out[t] = boys_one(tab, m, T[i]);
+}
+
+// J_ab blocks were accumulated for canonical pairs only where a != b needs the mirror; done inside the digestion.
+
+static int check_shells(const lx_shells_t *s, bool need_bf) {
+    if (!s) return LX_EINVAL;
+    if (s->nshell < 0) return LX_EINVAL;
+    if (s->nshell > 0 && (!s->L || !s->K || !s->prim_off || !s->center || !s->zeta || !s->coef)) return LX_EINVAL;
+    if (need_bf && s->nshell > 0 && !s->bf_off) return LX_EINVAL;
+    return LX_OK;
+}
+
+static int class_supported(int lx_, int la, int lb) {
+    return lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM;
+}
+
+static int launch_pair_data(const DevShells &prim, const int32_t *pair_list, int npair, int swapped,
+                            const long long *pd_off, int kstride, double *pd, cudaStream_t st) {
+    if (npair == 0) return LX_OK;
+    const int kiter = std::min(kstride, 32);
+    const long long total = (long long)npair * kiter;
+    const int threads = 256;
+    long long blocks = (total + threads - 1) / threads;
+    if (blocks > 148LL * 16) blocks = 148LL * 16;
+    pair_data_kernel<<<(unsigned)blocks, threads, 0, st>>>(prim, pair_list, npair, swapped, pd_off, kstride, kiter, pd);
+    g.launches++;
+    LX_CUDA(cudaGetLastError());
+    return LX_OK;
+}
+
+}  // namespace lx
+
+using namespace lx;
+
+// ================================================================================================ C ABI
+extern "C" {
+
+const char *lx_version(void) { return "lx3 0.1 sm_100a (coop kernels, Lx<=6, La,Lb<=4)"; }
+
+const char *lx_strerror(int status) {
+    switch (status) {
+        case LX_OK: return "success";
+        case LX_EINVAL: return "invalid argument";
+        case LX_EUNSUPPORTED: return "class outside the compiled range (Lx<=6, La,Lb<=4)";
+        case LX_ENOMEM: return "workspace too small";
+        case LX_ECUDA: return g.cuda_msg;
+        case LX_ENOTINIT: return "lx_init() has not been called";
+        default: return "unknown status";
+    }
+}
+
+int lx_init(int device) {
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g.ready && g.device == device) return LX_OK;
+    LX_CUDA(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    LX_CUDA(cudaGetDeviceProperties(&prop, device));
+    g.num_sms = prop.multiProcessorCount;
+    std::vector<double> tab;
+    boys_table_host(tab);
+    if (g.boys_tab) cudaFree(g.boys_tab);
+    LX_CUDA(cudaMalloc(&g.boys_tab, tab.size() * sizeof(double)));
+    LX_CUDA(cudaMemcpy(g.boys_tab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    g.device = device;
+    g.ready = true;
+    return LX_OK;
+}
+
+int lx_finalize(void) {
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g.boys_tab) cudaFree(g.boys_tab);
+    if (g.arena) cudaFree(g.arena);
+    if (g.pinned) cudaFreeHost(g.pinned);
+    g.boys_tab = nullptr;
+    g.arena = nullptr;
+    g.arena_bytes = 0;
+    g.pinned = nullptr;
+    g.pinned_bytes = 0;
+    g.ready = false;
+    return LX_OK;
+}
+
+int64_t lx_launch_count(void) { return (int64_t)g.launches.load(); }
+
+int lx_boys(const double *T, int n, int mmax, double *out, void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (n < 0 || mmax < 0 || mmax > BOYS_MMAX) return LX_EINVAL;
+    if (n == 0) return LX_OK;
+    if (!T || !out) return LX_EINVAL;
+    const long long total = (long long)n * (mmax + 1);
+    boys_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(g.boys_tab, T, n, mmax, out);
+    g.launches++;
+    LX_CUDA(cudaGetLastError());
+    return LX_OK;
+}
+
+size_t lx_eri3_workspace_bytes(int lx_, int la, int lb, int nx, int npair, int kmax_pair) {
+    (void)lx_; (void)la; (void)lb; (void)nx;
+    if (npair <= 0 || kmax_pair <= 0) return 256;
+    return (size_t)npair * (size_t)kmax_pair * 5 * sizeof(double) + 256;
+}
+
+int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim, const int32_t *x_idx,
+                  int nx, const int32_t *pair_idx, int npair, double *out, void *workspace, size_t workspace_bytes,
+                  void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (nx < 0 || npair < 0) return LX_EINVAL;
+    if (!class_supported(lx_, la, lb)) return LX_EUNSUPPORTED;
+    if (nx == 0 || npair == 0) return LX_OK;
+    int rc;
+    if ((rc = check_shells(aux, false)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, false)) != LX_OK) return rc;
+    if (!x_idx || !pair_idx || !out || !workspace) return LX_EINVAL;
+    // kmax_pair is not passed here: the workspace holds npair*kstride*5 doubles, so derive the stride from its size
+    const size_t avail = workspace_bytes >= 256 ? workspace_bytes - 256 : 0;
+    const long long kstride_ll = (long long)(avail / ((size_t)npair * 5 * sizeof(double)));
+    if (kstride_ll < 1) return LX_ENOMEM;
+    const int kstride = (int)std::min<long long>(kstride_ll, 1 << 20);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int swapped = la < lb ? 1 : 0;
+    const int cla = swapped ? lb : la, clb = swapped ? la : lb;
+    DevShells dprim = dev_view(prim), daux = dev_view(aux);
+    double *pd = reinterpret_cast<double *>(workspace);
+    // the stride must cover the largest K_a*K_b of the batch: checked on the host only through the documented
+    // contract lx_eri3_workspace_bytes(kmax_pair)
+    if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kstride, pd, st)) != LX_OK) return rc;
+    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr};
+    PairData pdat{pd, nullptr, kstride};
+    DfArgs df{nullptr, nullptr, 0};
+    cudaError_t e = k_launch[0][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
+    g.launches++;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return LX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ schedule (a0)
+struct lx_schedule {
+    struct AuxBucket {
+        int L, K;
+        std::vector<int32_t> ids;   // sorted by Q descending
+        std::vector<double> q;
+        int32_t *d_ids = nullptr;
+    };
+    struct PairBucket {
+        int la, lb;                 // la >= lb (pairs stored swapped if needed)
+        std::vector<int32_t> pairs; // [n][2]
+        std::vector<double> q;
+        std::vector<long long> pd_off;
+        int kmax = 1;
+        int32_t *d_pairs = nullptr;
+        long long *d_pd_off = nullptr;
+    };
+    struct Launch {
+        int ab, pb;                 // bucket indices
+        long long nsets;
+        long long *d_cum = nullptr;
+    };
+    std::vector<AuxBucket> aux_b;
+    std::vector<PairBucket> pair_b;
+    std::vector<Launch> launches;
+    long long prim_pairs = 0, nsets = 0, nints = 0;
+    int naux_bf = 0, nbf = 0;
+};
+
+int lx_schedule_destroy(lx_schedule_t *s) {
+    if (!s) return LX_OK;
+    for (auto &b : s->aux_b) if (b.d_ids) cudaFree(b.d_ids);
+    for (auto &b : s->pair_b) {
+        if (b.d_pairs) cudaFree(b.d_pairs);
+        if (b.d_pd_off) cudaFree(b.d_pd_off);
+    }
+    for (auto &l : s->launches) if (l.d_cum) cudaFree(l.d_cum);
+    delete s;
+    return LX_OK;
+}
+
+int lx_schedule_create(const lx_shells_t *aux, const lx_shells_t *prim, const double *q_aux, const double *q_pair,
+                       const int32_t *pair_idx, int npair, double tau, lx_schedule_t **out) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (!out) return LX_EINVAL;
+    *out = nullptr;
+    int rc;
+    if ((rc = check_shells(aux, true)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, true)) != LX_OK) return rc;
+    if (npair < 0 || (npair > 0 && !pair_idx)) return LX_EINVAL;
+    const bool screen = q_aux && q_pair;
+    for (int i = 0; i < aux->nshell; ++i) if (aux->L[i] < 0 || aux->L[i] > LX_MAX_L_AUX) return LX_EUNSUPPORTED;
+    for (int i = 0; i < prim->nshell; ++i) if (prim->L[i] < 0 || prim->L[i] > LX_MAX_L_PRIM) return LX_EUNSUPPORTED;
+    for (int p = 0; p < npair; ++p)
+        for (int k = 0; k < 2; ++k)
+            if (pair_idx[2 * p + k] < 0 || pair_idx[2 * p + k] >= prim->nshell) return LX_EINVAL;
+
+    lx_schedule *s = new (std::nothrow) lx_schedule();
+    if (!s) return LX_ENOMEM;
+    s->naux_bf = aux->nshell ? aux->bf_off[aux->nshell] : 0;
+    s->nbf = prim->nshell ? prim->bf_off[prim->nshell] : 0;
+
+    // aux buckets keyed by (L, K), each sorted by Q descending (ties by shell id → deterministic)
+    {
+        std::vector<int> order(aux->nshell);
+        for (int i = 0; i < aux->nshell; ++i) order[i] = i;
+        auto qa = [&](int i) { return screen ? q_aux[i] : 0.0; };
+        std::sort(order.begin(), order.end(), [&](int x, int y) {
+            if (aux->L[x] != aux->L[y]) return aux->L[x] < aux->L[y];
+            if (aux->K[x] != aux->K[y]) return aux->K[x] < aux->K[y];
+            if (qa(x) != qa(y)) return qa(x) > qa(y);
+            return x < y;
+        });
+        for (int i : order) {
+            if (s->aux_b.empty() || s->aux_b.back().L != aux->L[i] || s->aux_b.back().K != aux->K[i]) {
+                s->aux_b.emplace_back();
+                s->aux_b.back().L = aux->L[i];
+                s->aux_b.back().K = aux->K[i];
+            }
+            s->aux_b.back().ids.push_back(i);
+            s->aux_b.back().q.push_back(qa(i));
+        }
+    }
+    // pair buckets keyed by (La, Lb) with La >= Lb, ordered by K_a K_b then Q descending
+    {
+        struct P { int a, b, kab; double q; };
+        std::vector<P> ps(npair);
+        for (int p = 0; p < npair; ++p) {
+            int a = pair_idx[2 * p], b = pair_idx[2 * p + 1];
+            if (prim->L[a] < prim->L[b]) std::swap(a, b);
+            ps[p] = P{a, b, prim->K[a] * prim->K[b], screen ? q_pair[p] : 0.0};
+        }
+        std::sort(ps.begin(), ps.end(), [&](const P &x, const P &y) {
+            const int lax = prim->L[x.a], lbx = prim->L[x.b], lay = prim->L[y.a], lby = prim->L[y.b];
+            if (lax != lay) return lax < lay;
+            if (lbx != lby) return lbx < lby;
+            if (x.kab != y.kab) return x.kab < y.kab;
+            if (x.q != y.q) return x.q > y.q;
+            if (x.a != y.a) return x.a < y.a;
+            return x.b < y.b;
+        });
+        long long po = 0;
+        for (const P &p : ps) {
+            const int la = prim->L[p.a], lb = prim->L[p.b];
+            if (s->pair_b.empty() || s->pair_b.back().la != la || s->pair_b.back().lb != lb) {
+                s->pair_b.emplace_back();
+                s->pair_b.back().la = la;
+                s->pair_b.back().lb = lb;
+            }
+            auto &b = s->pair_b.back();
+            b.pairs.push_back(p.a);
+            b.pairs.push_back(p.b);
+            b.q.push_back(p.q);
+            b.pd_off.push_back(po);
+            b.kmax = std::max(b.kmax, p.kab);
+            po += p.kab;
+        }
+        s->prim_pairs = po;
+    }
+    // per class: Schwarz prefix lengths → cumulative set counts
+    for (size_t ib = 0; ib < s->pair_b.size(); ++ib) {
+        auto &pb = s->pair_b[ib];
+        const size_t np = pb.q.size();
+        for (size_t ia = 0; ia < s->aux_b.size(); ++ia) {
+            auto &ab = s->aux_b[ia];
+            std::vector<long long> cum(np + 1, 0);
+            for (size_t p = 0; p < np; ++p) {
+                long long n = (long long)ab.ids.size();
+                if (screen) {
+                    // aux q sorted descending: survivors (q_x*q_p >= tau, the same double expression the oracle
+                    // uses) are a prefix; binary search for its length
+                    size_t lo = 0, hi = ab.ids.size();
+                    while (lo < hi) {
+                        const size_t mid = (lo + hi) / 2;
+                        if (ab.q[mid] * pb.q[p] < tau) hi = mid; else lo = mid + 1;
+                    }
+                    n = (long long)lo;
+                }
+                cum[p + 1] = cum[p] + n;
+            }
+            if (cum[np] == 0) continue;
+            lx_schedule::Launch l;
+            l.ab = (int)ia;
+            l.pb = (int)ib;
+            l.nsets = cum[np];
+            if (cudaMalloc(&l.d_cum, cum.size() * sizeof(long long)) != cudaSuccess ||
+                cudaMemcpy(l.d_cum, cum.data(), cum.size() * sizeof(long long), cudaMemcpyHostToDevice) != cudaSuccess) {
+                lx_schedule_destroy(s);
+                return cuda_fail(cudaGetLastError());
+            }
+            s->launches.push_back(l);
+            s->nsets += l.nsets;
+            s->nints += l.nsets * nc(ab.L) * nc(pb.la) * nc(pb.lb);
+        }
+    }
+    for (auto &b : s->aux_b) {
+        if (cudaMalloc(&b.d_ids, b.ids.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMemcpy(b.d_ids, b.ids.data(), b.ids.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess) {
+            lx_schedule_destroy(s);
+            return cuda_fail(cudaGetLastError());
+        }
+    }
+    for (auto &b : s->pair_b) {
+        if (cudaMalloc(&b.d_pairs, b.pairs.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMemcpy(b.d_pairs, b.pairs.data(), b.pairs.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMalloc(&b.d_pd_off, b.pd_off.size() * sizeof(long long)) != cudaSuccess ||
+            cudaMemcpy(b.d_pd_off, b.pd_off.data(), b.pd_off.size() * sizeof(long long), cudaMemcpyHostToDevice) != cudaSuccess) {
+            lx_schedule_destroy(s);
+            return cuda_fail(cudaGetLastError());
+        }
+    }
+    *out = s;
+    return LX_OK;
+}
+
+int64_t lx_schedule_num_sets(const lx_schedule_t *s) { return s ? s->nsets : 0; }
+int64_t lx_schedule_num_integrals(const lx_schedule_t *s) { return s ? s->nints : 0; }
+size_t lx_df_workspace_bytes(const lx_schedule_t *s) {
+    return s ? (size_t)s->prim_pairs * 5 * sizeof(double) + 256 : 256;
+}
+
+static int df_run(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, int mode, const DfArgs &df,
+                  void *workspace, size_t workspace_bytes, cudaStream_t st) {
+    if (workspace_bytes < lx_df_workspace_bytes(s)) return LX_ENOMEM;
+    DevShells dprim = dev_view(prim), daux = dev_view(aux);
+    double *pd = reinterpret_cast<double *>(workspace);
+    int rc;
+    for (const auto &pb : s->pair_b)
+        if ((rc = launch_pair_data(dprim, pb.d_pairs, (int)pb.q.size(), 0, pb.d_pd_off, pb.kmax, pd, st)) != LX_OK) return rc;
+    for (const auto &l : s->launches) {
+        const auto &ab = s->aux_b[l.ab];
+        const auto &pb = s->pair_b[l.pb];
+        SetMap map{l.nsets, (int)ab.ids.size(), (int)pb.q.size(), ab.d_ids, pb.d_pairs, l.d_cum};
+        PairData pdat{pd, pb.d_pd_off, pb.kmax};
+        cudaError_t e = k_launch[mode][ab.L](pb.la, pb.lb, map, daux, dprim, pdat, g.boys_tab, nullptr, 0, df, g.num_sms, st);
+        g.launches++;
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return LX_OK;
+}
+
+int lx_df_gamma(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *D, int ldD,
+                double *gamma, void *workspace, size_t workspace_bytes, void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (!s || !D || !gamma || !workspace) return LX_EINVAL;
+    int rc;
+    if ((rc = check_shells(aux, true)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, true)) != LX_OK) return rc;
+    if (ldD < s->nbf) return LX_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    LX_CUDA(cudaMemsetAsync(gamma, 0, (size_t)s->naux_bf * sizeof(double), st));
+    DfArgs df{D, gamma, ldD};
+    return df_run(s, aux, prim, 1, df, workspace, workspace_bytes, st);
+}
+
+int lx_df_J(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *d, double *J,
+            int ldJ, void *workspace, size_t workspace_bytes, void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (!s || !d || !J || !workspace) return LX_EINVAL;
+    int rc;
+    if ((rc = check_shells(aux, true)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, true)) != LX_OK) return rc;
+    if (ldJ < s->nbf) return LX_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    LX_CUDA(cudaMemsetAsync(J, 0, (size_t)s->nbf * (size_t)ldJ * sizeof(double), st));
+    DfArgs df{d, J, ldJ};
+    return df_run(s, aux, prim, 2, df, workspace, workspace_bytes, st);
+}
+
+// ------------------------------------------------------------------------------------------------ host-buffer path
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int lx_eri3_batch_host(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim,
+                       const int32_t *x_idx, int nx, const int32_t *pair_idx, int npair, double *out) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (nx < 0 || npair < 0) return LX_EINVAL;
+    if (!class_supported(lx_, la, lb)) return LX_EUNSUPPORTED;
+    if (nx == 0 || npair == 0) return LX_OK;
+    int rc;
+    if ((rc = check_shells(aux, false)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, false)) != LX_OK) return rc;
+    if (!x_idx || !pair_idx || !out) return LX_EINVAL;
+    int kmax = 1;
+    for (int p = 0; p < npair; ++p) kmax = std::max(kmax, prim->K[pair_idx[2 * p]] * prim->K[pair_idx[2 * p + 1]]);
+    const size_t nint = (size_t)npair * nx * nc(lx_) * nc(la) * nc(lb);
+    const size_t ws = lx_eri3_workspace_bytes(lx_, la, lb, nx, npair, kmax);
+    auto tab_bytes = [](const lx_shells_t *s, size_t *np) {
+        *np = (size_t)s->prim_off[s->nshell];
+        return 3 * align256((size_t)(s->nshell + 1) * 4) + align256((size_t)s->nshell * 24) + 2 * align256(*np * 8);
+    };
+    size_t npx, npp;
+    const size_t in_bytes = tab_bytes(aux, &npx) + tab_bytes(prim, &npp) + align256((size_t)nx * 4) + align256((size_t)npair * 8);
+    const size_t total = in_bytes + align256(ws) + align256(nint * 8);
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g.arena_bytes < total) {
+        if (g.arena) cudaFree(g.arena);
+        g.arena = nullptr;
+        g.arena_bytes = 0;
+        LX_CUDA(cudaMalloc(&g.arena, total));
+        g.arena_bytes = total;
+    }
+    char *base = reinterpret_cast<char *>(g.arena);
+    size_t o = 0;
+    cudaStream_t st = 0;
+    auto put = [&](const void *src, size_t bytes) -> void * {
+        void *d = base + o;
+        cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st);
+        o += align256(bytes);
+        return d;
+    };
+    auto put_tab = [&](const lx_shells_t *s, size_t np, lx_shells_t *d) {
+        d->nshell = s->nshell;
+        d->L = (const int32_t *)put(s->L, (size_t)s->nshell * 4);
+        d->K = (const int32_t *)put(s->K, (size_t)s->nshell * 4);
+        d->prim_off = (const int32_t *)put(s->prim_off, (size_t)(s->nshell + 1) * 4);
+        d->center = (const double *)put(s->center, (size_t)s->nshell * 24);
+        d->zeta = (const double *)put(s->zeta, np * 8);
+        d->coef = (const double *)put(s->coef, np * 8);
+        d->bf_off = nullptr;
+    };
+    lx_shells_t daux, dprim;
+    put_tab(aux, npx, &daux);
+    put_tab(prim, npp, &dprim);
+    const int32_t *dx = (const int32_t *)put(x_idx, (size_t)nx * 4);
+    const int32_t *dp = (const int32_t *)put(pair_idx, (size_t)npair * 8);
+    void *dws = base + o;
+    o += align256(ws);
+    double *dout = reinterpret_cast<double *>(base + o);
+    LX_CUDA(cudaGetLastError());
+    rc = lx_eri3_batch(lx_, la, lb, &daux, &dprim, dx, nx, dp, npair, dout, dws, ws, st);
+    if (rc != LX_OK) return rc;
+    LX_CUDA(cudaMemcpyAsync(out, dout, nint * 8, cudaMemcpyDeviceToHost, st));
+    LX_CUDA(cudaStreamSynchronize(st));
+    return LX_OK;
+}
+
+}  // extern "C"

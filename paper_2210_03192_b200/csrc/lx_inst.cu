@@ -1,0 +1,34 @@
+// lx_inst.cu — instantiates the class kernels for one aux angular momentum (INST_LX) and one digestion mode
+// (INST_MODE: 0 store, 1 γ, 2 J).  Compiled once per (INST_LX, INST_MODE); no code generator: every class is a
+// template instantiation.
+#include "lx_coop.cuh"
+#include "lx_dispatch.h"
+
+#ifndef INST_LX
+#error "compile with -DINST_LX=<0..6> -DINST_MODE=<0..2>"
+#endif
+
+namespace lx {
+
+#define LX_CASE(LA_, LB_)                                                                                        \
+    case LA_ * 8 + LB_:                                                                                           \
+        return coop_launch<INST_LX, LA_, LB_, INST_MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+
+#define LX_CAT_(a, b, c, d) a##b##c##d
+#define LX_CAT(a, b, c, d) LX_CAT_(a, b, c, d)
+
+cudaError_t LX_CAT(launch_lx, INST_LX, _mode, INST_MODE)(int la, int lb, const SetMap &map, const DevShells &aux,
+                                                           const DevShells &prim, const PairData &pdat,
+                                                           const double *boys_tab, double *out, int swapped,
+                                                           const DfArgs &df, int num_sms, cudaStream_t stream) {
+    switch (la * 8 + lb) {
+        LX_CASE(0, 0)
+        LX_CASE(1, 0) LX_CASE(1, 1)
+        LX_CASE(2, 0) LX_CASE(2, 1) LX_CASE(2, 2)
+        LX_CASE(3, 0) LX_CASE(3, 1) LX_CASE(3, 2) LX_CASE(3, 3)
+        LX_CASE(4, 0) LX_CASE(4, 1) LX_CASE(4, 2) LX_CASE(4, 3) LX_CASE(4, 4)
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace lx

@@ -1,0 +1,203 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star): integrals max-abs <= 1e-12 x batch max |integral|;
+gamma, J relative Frobenius <= 1e-11.
+"""
+import numpy as np
+import pytest
+
+import lx_inputs as gen
+from helpers import table
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def lx():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2210_03192_b200 import lx as _lx
+    _lx.lx_init(0)
+    return _lx
+
+
+def _run(lx, cfg):
+    import torch
+    aux, prim = lx.DeviceShells(cfg["aux"]), lx.DeviceShells(cfg["prim"])
+    out = lx.lx_eri3_batch(cfg["lx"], cfg["la"], cfg["lb"], aux, prim, cfg["x_idx"], cfg["pair_idx"])
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _check(got, ref, tol=TOL):
+    assert got.shape == ref.shape
+    scale = np.max(np.abs(ref))
+    err = np.max(np.abs(got - ref))
+    assert np.isfinite(got).all()
+    assert err <= tol * scale, f"max-abs err {err:.3e} vs scale {scale:.3e} (ratio {err / scale:.2e})"
+
+
+def test_boys_sweep(lx, oracle):
+    """Device Boys vs oracle Boys on a dense sweep T in [0,200], m <= 18 (reading G12): <= 4 ulp relative."""
+    import torch
+    rng = np.random.default_rng(1)
+    T = np.concatenate([np.linspace(0, 200, 4001), rng.uniform(0, 90, 4000), [83.999999, 84.0, 84.000001, 1e-300, 1e-9],
+                        np.arange(0, 1346) / 16.0 + 1.0 / 32.0])
+    got = lx.lx_boys(torch.from_numpy(T).cuda(), 18).cpu().numpy()
+    ref = np.stack([oracle.boys_ld(18, float(t)).astype(np.float64) for t in T])
+    rel = np.abs(got - ref) / ref
+    ulp = 2.2204e-16
+    tab = T < 84.0
+    # table + degree-7 Taylor region: <= 4 ulp; asymptotic region: a product of m+4 correctly rounded factors,
+    # <= 8 ulp
+    assert rel[tab].max() <= 4 * ulp, (rel[tab].max() / ulp, T[tab][np.unravel_index(rel[tab].argmax(), rel[tab].shape)[0]])
+    assert rel[~tab].max() <= 8 * ulp, (rel[~tab].max() / ulp, T[~tab][np.unravel_index(rel[~tab].argmax(), rel[~tab].shape)[0]])
+
+
+def test_config1_full_tensor(lx, oracle):
+    cfg = gen.config1()
+    ref = oracle.eri3_batch(2, 1, 1, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"])
+    got = _run(lx, cfg)
+    assert got.shape == (64, 32, 6, 3, 3)
+    _check(got, ref)
+
+
+@pytest.mark.parametrize("lxa", range(5))
+def test_config2_class_sweep_reduced(lx, oracle, lxa):
+    """All 9 (la,lb) of config 2 for one lx (mirrored la<lb classes exercise the swap path); K_total = 9; sizes span
+    several blocks and a ragged tail."""
+    for la in range(3):
+        for lb in range(3):
+            cfg = gen.config2(lxa, la, lb, npair=37, nx=19)
+            ref = oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"])
+            _check(_run(lx, cfg), ref)
+
+
+@pytest.mark.parametrize("cls", gen.CONFIG3_CLASSES)
+def test_config3_high_L_reduced(lx, oracle, cls):
+    lxa, la, lb, k = cls
+    cfg = gen.config3(lxa, la, lb, kprim=k, npair=11, nx=7)
+    ref = oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"])
+    _check(_run(lx, cfg), ref)
+
+
+@pytest.mark.parametrize("lxa", range(7))
+def test_every_compiled_class_tiny(lx, oracle, lxa):
+    """Every class in the compiled range (Lx <= 6; La, Lb <= 4, both orders), contracted aux shells included."""
+    rng = np.random.default_rng(100 + lxa)
+    for la in range(5):
+        for lb in range(5):
+            shells = []
+            for l in (la, lb, la, lb):
+                k = int(rng.integers(1, 3))
+                z = np.exp(rng.uniform(np.log(0.2), np.log(3.0), k))
+                shells.append((l, rng.uniform(0, 3, 3), z, rng.uniform(0.3, 1.0, k) * gen.prim_norm(z, l)))
+            prim = table(shells)
+            xs = []
+            for _ in range(2):
+                k = int(rng.integers(1, 3))
+                z = np.exp(rng.uniform(np.log(0.2), np.log(3.0), k))
+                xs.append((lxa, rng.uniform(0, 3, 3), z, rng.uniform(0.3, 1.0, k) * gen.prim_norm(z, lxa)))
+            aux = table(xs)
+            cfg = dict(lx=lxa, la=la, lb=lb, aux=aux, prim=prim, x_idx=np.array([1, 0], np.int32),
+                       pair_idx=np.array([[0, 1], [2, 3], [2, 1]], np.int32))
+            ref = oracle.eri3_batch(lxa, la, lb, aux, prim, cfg["x_idx"], cfg["pair_idx"])
+            _check(_run(lx, cfg), ref)
+
+
+def test_degenerate_geometry(lx, oracle):
+    """A = B, P = C (T = 0), all centres equal, same shell twice in a pair (reading G15)."""
+    z = np.zeros(3)
+    c1 = np.array([0.4, -0.2, 0.9])
+    prim = table([(2, z, [1.1, 0.3], [0.5, 0.8]), (1, z, [0.7], [1.0]), (2, c1, [0.9], [1.0]), (1, c1 + 1.0, [2.0], [0.7])])
+    aux = table([(3, z, [0.6], [1.0]), (3, c1, [1.4, 0.2], [0.3, 0.9])])
+    pairs = np.array([[0, 0], [2, 2], [0, 2]], np.int32)
+    ref = oracle.eri3_batch(3, 2, 2, aux, prim, [0, 1], pairs)
+    got = _run(lx, dict(lx=3, la=2, lb=2, aux=aux, prim=prim, x_idx=np.array([0, 1], np.int32), pair_idx=pairs))
+    _check(got, ref)
+    pairs = np.array([[0, 1], [2, 1], [2, 3]], np.int32)
+    ref = oracle.eri3_batch(3, 2, 1, aux, prim, [0, 1], pairs)
+    got = _run(lx, dict(lx=3, la=2, lb=1, aux=aux, prim=prim, x_idx=np.array([0, 1], np.int32), pair_idx=pairs))
+    _check(got, ref)
+
+
+def test_large_T_and_far_field(lx, oracle):
+    """Tight exponents far apart: T beyond the Boys table (asymptotic branch) and underflowing overlaps."""
+    prim = table([(1, [0, 0, 0], [9.0], [1.0]), (2, [0.5, 0, 0], [7.0], [1.0])])
+    aux = table([(2, [0, 0, 30.0], [8.0], [1.0]), (2, [0.1, 0.2, 0.3], [8.0], [1.0]), (2, [0, 4.5, 0.0], [5.0], [1.0])])
+    cfg = dict(lx=2, la=1, lb=2, aux=aux, prim=prim, x_idx=np.arange(3, dtype=np.int32), pair_idx=np.array([[0, 1]], np.int32))
+    ref = oracle.eri3_batch(2, 1, 2, aux, prim, cfg["x_idx"], cfg["pair_idx"])
+    got = _run(lx, cfg)
+    for x in range(3):   # per aux shell: scales differ by many orders of magnitude
+        _check(got[:, x], ref[:, x])
+
+
+def test_empty_and_errors(lx):
+    import torch
+    cfg = gen.config1(npair=2, nx=2)
+    aux, prim = lx.DeviceShells(cfg["aux"]), lx.DeviceShells(cfg["prim"])
+    out = lx.lx_eri3_batch(2, 1, 1, aux, prim, np.zeros(0, np.int32), cfg["pair_idx"])
+    assert out.numel() == 0
+    out = lx.lx_eri3_batch(2, 1, 1, aux, prim, cfg["x_idx"], np.zeros((0, 2), np.int32))
+    assert out.numel() == 0
+    with pytest.raises(lx.LxError) as e:
+        lx.lx_eri3_batch(7, 1, 1, aux, prim, cfg["x_idx"], cfg["pair_idx"],
+                         out=torch.empty(10, dtype=torch.float64, device="cuda"))
+    assert e.value.status == lx.LX_EUNSUPPORTED
+    with pytest.raises(lx.LxError) as e:
+        lx.lx_eri3_batch(2, 1, 1, aux, prim, cfg["x_idx"], cfg["pair_idx"],
+                         workspace=torch.empty(8, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == lx.LX_ENOMEM
+
+
+def test_host_buffer_path(lx, oracle):
+    cfg = gen.config2(2, 1, 0, npair=9, nx=5)
+    ref = oracle.eri3_batch(2, 1, 0, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"])
+    got = lx.lx_eri3_batch_host(2, 1, 0, lx.HostShells(cfg["aux"]), lx.HostShells(cfg["prim"]), cfg["x_idx"], cfg["pair_idx"])
+    _check(got, ref)
+
+
+def _df_small(seed=21, natom=5):
+    rng = np.random.default_rng(seed)
+    prim, aux = gen._cluster(rng, natom, 7.0, gen._PRIM4, gen._AUX4)
+    nbf, naux = prim.nbf, aux.nbf
+    Cm = rng.normal(0, 1 / np.sqrt(nbf), size=(nbf, nbf // 4))
+    return prim, aux, Cm @ Cm.T, rng.normal(size=naux)
+
+
+@pytest.mark.parametrize("tau", [1e-12, 1e-5])
+def test_df_gamma_J_small_cluster(lx, oracle, tau):
+    import torch
+    prim, aux, D, d = _df_small()
+    pairs = gen.unique_pairs(prim.nshell)
+    qx, qp = oracle.schwarz_aux(aux), oracle.schwarz_pair(prim, pairs)
+    g_ref, J_ref, nsets, nints = oracle.df_gamma_J(aux, prim, pairs, qx, qp, tau, D=D, d=d)
+    ha, hp = lx.HostShells(aux), lx.HostShells(prim)
+    sched = lx.Schedule(ha, hp, qx, qp, pairs, tau)
+    assert sched.num_sets == nsets and sched.num_integrals == nints      # integer work: bit-exact
+    da, dp = lx.DeviceShells(ha), lx.DeviceShells(hp)
+    gamma = lx.lx_df_gamma(sched, da, dp, torch.from_numpy(D).cuda())
+    J = lx.lx_df_J(sched, da, dp, torch.from_numpy(d).cuda())
+    torch.cuda.synchronize()
+    gamma, J = gamma.cpu().numpy(), J.cpu().numpy()
+    assert np.linalg.norm(gamma - g_ref) <= 1e-11 * np.linalg.norm(g_ref)
+    assert np.linalg.norm(J - J_ref) <= 1e-11 * np.linalg.norm(J_ref)
+    assert abs(gamma @ d - np.sum(J * D)) <= 1e-10 * abs(gamma @ d)
+
+
+def test_df_no_screening_and_subset_pairs(lx, oracle):
+    import torch
+    prim, aux, D, d = _df_small(seed=22, natom=3)
+    pairs = gen.unique_pairs(prim.nshell)[::3]
+    g_ref, J_ref, nsets, _ = oracle.df_gamma_J(aux, prim, pairs, None, None, 0.0, D=D, d=d)
+    ha, hp = lx.HostShells(aux), lx.HostShells(prim)
+    sched = lx.Schedule(ha, hp, None, None, pairs, 0.0)
+    assert sched.num_sets == nsets == len(pairs) * aux.nshell
+    da, dp = lx.DeviceShells(ha), lx.DeviceShells(hp)
+    gamma = lx.lx_df_gamma(sched, da, dp, torch.from_numpy(D).cuda()).cpu().numpy()
+    J = lx.lx_df_J(sched, da, dp, torch.from_numpy(d).cuda()).cpu().numpy()
+    assert np.linalg.norm(gamma - g_ref) <= 1e-11 * np.linalg.norm(g_ref)
+    assert np.linalg.norm(J - J_ref) <= 1e-11 * np.linalg.norm(J_ref)
