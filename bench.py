@@ -1,0 +1,291 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the whole hot path on BASELINE.json configs[1] (class sweep).
+
+One "step" = one pass of lx_eri3_batch over all 45 (Lx|LaLb) classes of config 2 (Lx 0..4; La,Lb 0..2; primary K=3,
+aux K=1 → K_total = 9; 1024 shell pairs x 256 aux shells per class = 262 144 shell-sets per class), i.e. Boys → VRR1 →
+VRR2 → contraction → HRR → store for 11.8 M shell-sets / 0.92 G integrals (7.3 GB of output), inputs resident in HBM.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Prints ONE JSON line (contract in the task statement).  `--impl reference` times the CPU oracle (as it stands) on the
+host cores for the same metric on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import lx_inputs as gen  # noqa: E402
+
+METRIC = "3-center integrals/sec (class sweep, config 2)"
+UNIT = "integrals/s"
+WORKLOAD = "configs[1]: 45 classes (Lx 0..4 | La,Lb 0..2), K_total=9, 1024 pairs x 256 aux per class"
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk/SM x 2 x sm_max_mhz
+# SURVEY.md §8(d) table, flops per shell-set at K = 9 for the classes it lists
+SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
+                        (4, 1, 1): 29322, (4, 2, 2): 111054}
+
+
+def ncart(l):
+    return (l + 1) * (l + 2) // 2
+
+
+def nint_set(c):
+    return ncart(c[0]) * ncart(c[1]) * ncart(c[2])
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(classes, npair_s, nx_s, seed):
+    """Oracle (double instantiation, OpenMP over pairs) on the first npair_s pairs x nx_s aux shells of every class."""
+    import oracle
+    oracle.build()
+    total_int, total_t = 0, 0.0
+    for c in classes:
+        cfg = gen.config2(*c, seed=seed)
+        t0 = time.perf_counter()
+        o = oracle.eri3_batch(c[0], c[1], c[2], cfg["aux"], cfg["prim"], cfg["x_idx"][:nx_s], cfg["pair_idx"][:npair_s], real="d")
+        total_t += time.perf_counter() - t0
+        total_int += o.size
+    return total_int, total_t, oracle.max_threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    classes = gen.CONFIG2_CLASSES
+    npair_s, nx_s = 32, 256
+    times = []
+    nint = 0
+    for it in range(args.warmup + args.steps):
+        n, t, cores = oracle_sample(classes, npair_s, nx_s, seed=2)
+        nint = n
+        if it >= args.warmup:
+            times.append(t)
+    tot = sum(times)
+    val = nint * len(times) / tot
+    sample = f"first {npair_s} pairs x {nx_s} aux shells of each of the 45 classes per step ({nint} integrals)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--npair", type=int, default=1024, help="pairs per class (default = config 2)")
+    ap.add_argument("--nx", type=int, default=256, help="aux shells per class (default = config 2)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2210_03192_b200 import lx, costmodel
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    lx.lx_init(local)
+
+    # ---- inputs: one full config-2 batch per rank (weak scaling: independent shell-sets, no collective) --------
+    classes = gen.CONFIG2_CLASSES
+    seed = 2 + 1000 * rank
+    host, devs = {}, {}
+    for c in classes:
+        cfg = gen.config2(*c, npair=args.npair, nx=args.nx, seed=seed)
+        ha, hp = lx.HostShells(cfg["aux"]), lx.HostShells(cfg["prim"])
+        host[c] = (ha, hp, cfg["x_idx"], cfg["pair_idx"])
+        devs[c] = (lx.DeviceShells(ha, dev), lx.DeviceShells(hp, dev),
+                   torch.from_numpy(cfg["x_idx"]).to(dev), torch.from_numpy(cfg["pair_idx"]).to(dev))
+    nsets = args.npair * args.nx
+    max_int = max(nint_set(c) for c in classes) * nsets
+    out = torch.empty(max_int, dtype=torch.float64, device=dev)
+    ws = torch.empty(lx.lx_eri3_workspace_bytes(0, 0, 0, args.nx, args.npair, 9), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    ints_per_step = sum(nint_set(c) for c in classes) * nsets
+    probe = lx.lx_fp64_probe(20000)
+
+    def one_step(evs=None):
+        for i, c in enumerate(classes):
+            da, dp, dx, dpr = devs[c]
+            if evs is not None:
+                evs[i][0].record()
+            lx.lx_eri3_batch(c[0], c[1], c[2], da, dp, dx, dpr, out=out, workspace=ws, kmax=9)
+            if evs is not None:
+                evs[i][1].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = lx.lx_launch_count()
+    step_ms = []
+    class_ms = np.zeros(len(classes))
+    for _ in range(args.steps):
+        flush.fill_(1)                      # L2 flush between timed iterations (outside the timed interval)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in classes]
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        s0.record()
+        one_step(evs)
+        s1.record()
+        barrier()
+        step_ms.append(s0.elapsed_time(s1))
+        class_ms += np.array([a.elapsed_time(b) for a, b in evs])
+    launches = lx.lx_launch_count() - launches0
+    clocks = sampler.stop()
+    class_ms /= args.steps
+    t_total = torch.tensor([sum(step_ms) * 1e-3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
+    t_total = float(t_total.item())
+    value = world * ints_per_step * args.steps / t_total
+
+    # ---- end to end: host buffers through the C ABI, H2D of inputs and D2H of the result inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        pin = torch.empty(max_int, dtype=torch.float64).pin_memory()
+        pin_np = pin.numpy()
+        h2d = sum(h[0].nbytes() + h[1].nbytes() + h[2].nbytes + h[3].nbytes for h in host.values())
+        d2h = ints_per_step * 8
+
+        def e2e_step():
+            for c in classes:
+                ha, hp, xi, pi = host[c]
+                n = nint_set(c) * nsets
+                lx.lx_eri3_batch_host(c[0], c[1], c[2], ha, hp, xi, pi,
+                                      out=pin_np[:n].reshape(args.npair, args.nx, ncart(c[0]), ncart(c[1]), ncart(c[2])))
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        nrep = max(1, min(args.steps, 3))
+        for _ in range(nrep):
+            e2e_step()
+        barrier()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * ints_per_step * nrep / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": nrep}
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel (the class with the largest share of the step) -----------------------
+        i_top = int(np.argmax(class_ms))
+        c_top = classes[i_top]
+        canon = (c_top[0], max(c_top[1:]), min(c_top[1:]))
+        fl_min = costmodel.flops_per_set(*c_top, 9)
+        fl_set = SURVEY_FLOPS_PER_SET.get(canon, fl_min)
+        t_top = class_ms[i_top] * 1e-3
+        achieved = fl_set * nsets / t_top / 1e12
+        roofline = {"bound": "alu", "kernel": f"coop_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
+                    "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+                    "traffic": None, "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
+                    "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
+                    "flops_per_set_min_model": fl_min, "kernel_ms": class_ms[i_top],
+                    "share_of_step": float(class_ms[i_top] / class_ms.sum()),
+                    "hbm_write_gbs": nint_set(c_top) * 8 * nsets / t_top / 1e9}
+        cpu = None
+        if world == 1 and not args.no_cpu:
+            # bounded sample: calibrate on 16 pairs per class, then size the sample for ~15 s of CPU work
+            _, t_cal, _ = oracle_sample(classes, 16, 256, seed=2)
+            npair_s, nx_s = int(min(args.npair, max(16, 16 * 15.0 / max(t_cal, 1e-3)))), min(256, args.nx)
+            n, t, cores = oracle_sample(classes, npair_s, nx_s, seed=2)
+            cpu = {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"first {npair_s} pairs x {nx_s} aux shells of each of the 45 classes ({n} integrals, {t:.1f} s)"}
+        per_class = {f"({c[0]}|{c[1]}{c[2]})": round(float(nint_set(c) * nsets / (m * 1e-3)), 1) for c, m in zip(classes, class_ms)}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": WORKLOAD if (args.npair, args.nx) == (1024, 256) else f"reduced config 2: {args.npair} pairs x {args.nx} aux",
+                           "shell_sets_per_step": nsets * len(classes) * world, "integrals_per_step": ints_per_step * world,
+                           "l2": "flushed between timed steps (256 MiB fill, outside the timed interval); each step also writes "
+                                 f"{ints_per_step * 8 / 1e9:.1f} GB of output",
+                           "parallelism": f"{world} x independent batch (no collective)"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+                "shell_sets_per_s": value / ints_per_step * nsets * len(classes),
+                "integrals_per_s_per_class": per_class}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -132,6 +132,11 @@ int lx_eri3_batch_host(int lx, int la, int lb, const lx_shells_t *aux_host, cons
  * exported for the accuracy sweep.  T [n] and out [n*(mmax+1)] are device pointers; mmax <= 18. */
 int lx_boys(const double *T, int n, int mmax, double *out, void *stream);
 
+/* Measurement helper: sustained FP64 FMA rate of the device (TFLOP/s, FMA = 2 flops) from a register-resident chain
+ * kernel (8 independent DFMA chains per thread, 8 blocks x 256 threads per SM, `iters` x 64 FMAs per thread), best of
+ * 5 timed launches.  This is the measured denominator of the FP64-pipe roofline; synchronises. */
+int lx_fp64_probe(int iters, double *tflops_host);
+
 /* Number of kernel launches the library has issued since lx_init (for the bench's `gpu_launches` claim). */
 int64_t lx_launch_count(void);
 

@@ -110,7 +110,20 @@ __global__ void boys_kernel(const double *__restrict__ tab, const double *__rest
     out[t] = boys_one(tab, m, T[i]);
 }
 
-// J_ab blocks were accumulated for canonical pairs only where a != b needs the mirror; done inside the digestion.
+// FP64 FMA throughput probe: 8 independent DFMA chains per thread (roofline denominator of the ALU-bound classes).
+__global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double seed, double *__restrict__ sink) {
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+    }
+    const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 123.456) sink[0] = r;
+}
 
 static int check_shells(const lx_shells_t *s, bool need_bf) {
     if (!s) return LX_EINVAL;
@@ -191,6 +204,35 @@ int lx_finalize(void) {
 }
 
 int64_t lx_launch_count(void) { return (int64_t)g.launches.load(); }
+
+int lx_fp64_probe(int iters, double *tflops_host) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (iters <= 0 || !tflops_host) return LX_EINVAL;
+    double *sink = nullptr;
+    LX_CUDA(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    LX_CUDA(cudaEventCreate(&e0));
+    LX_CUDA(cudaEventCreate(&e1));
+    const int blocks = g.num_sms * 8, threads = 256;
+    dfma_probe_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, sink);  // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0);
+        dfma_probe_kernel<<<blocks, threads>>>(iters, 1.0, sink);
+        cudaEventRecord(e1);
+        LX_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 2.0 * 64.0 * (double)iters * (double)blocks * threads;
+        best = std::max(best, fl / (ms * 1e-3) * 1e-12);
+    }
+    g.launches += 6;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    *tflops_host = best;
+    return LX_OK;
+}
 
 int lx_boys(const double *T, int n, int mmax, double *out, void *stream) {
     if (!g.ready) return LX_ENOTINIT;

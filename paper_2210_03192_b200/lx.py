@@ -22,7 +22,7 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
-           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count"]
+           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe"]
 
 
 class lx_shells_t(C.Structure):
@@ -248,3 +248,10 @@ def lx_boys(T, mmax, stream=None):
     out = torch.empty((T.numel(), mmax + 1), dtype=torch.float64, device=T.device)
     _check(_lib.lx_boys(T.data_ptr(), T.numel(), mmax, out.data_ptr(), _stream_ptr(stream)))
     return out
+
+
+def lx_fp64_probe(iters=20000):
+    """Measured FP64 FMA rate of the device in TFLOP/s (register-resident DFMA chains)."""
+    v = C.c_double(0.0)
+    _check(_lib.lx_fp64_probe(C.c_int(iters), C.byref(v)))
+    return float(v.value)
