@@ -1,7 +1,7 @@
 // lx_inst.cu — instantiates the class kernels for one aux angular momentum (INST_LX) and one digestion mode
 // (INST_MODE: 0 store, 1 γ, 2 J).  Compiled once per (INST_LX, INST_MODE); no code generator: every class is a
 // template instantiation.
-#include "lx_coop.cuh"
+#include "lx_group.cuh"
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
@@ -12,7 +12,7 @@ namespace lx {
 
 #define LX_CASE(LA_, LB_)                                                                                        \
     case LA_ * 8 + LB_:                                                                                           \
-        return coop_launch<INST_LX, LA_, LB_, INST_MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+        return group_launch<INST_LX, LA_, LB_, INST_MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
 
 #define LX_CAT_(a, b, c, d) a##b##c##d
 #define LX_CAT(a, b, c, d) LX_CAT_(a, b, c, d)
