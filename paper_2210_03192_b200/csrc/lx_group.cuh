@@ -37,6 +37,41 @@ __host__ __device__ constexpr int pow2ceil(int x) {
     return p;
 }
 
+// Which auxiliary orders m of [·|c]^(m) are actually reachable from the targets [·|c]^(0), |c| = LX, when the ket is
+// lowered along the axis with the smallest positive power (the DAG of reading G4): inclusive range lo..hi per ket
+// component, hi < lo = never needed.  Evaluated at compile time; the kernel skips everything outside.
+struct KetNeed {
+    int lo[LX_MAX_L_AUX + 1][nc(LX_MAX_L_AUX)];
+    int hi[LX_MAX_L_AUX + 1][nc(LX_MAX_L_AUX)];
+};
+constexpr KetNeed ket_need(int LX) {
+    KetNeed t{};
+    for (int k = 0; k <= LX_MAX_L_AUX; ++k)
+        for (int c = 0; c < nc(LX_MAX_L_AUX); ++c) { t.lo[k][c] = 99; t.hi[k][c] = -1; }
+    for (int c = 0; c < nc(LX); ++c) { t.lo[LX][c] = 0; t.hi[LX][c] = 0; }
+    for (int k = LX; k >= 1; --k)
+        for (int cc = 0; cc < nc(k); ++cc) {
+            if (t.hi[k][cc] < t.lo[k][cc]) continue;
+            const uint32_t ck = cart_entry(off(k) + cc);
+            const int dir = ck >> 24, ci = (ck >> (8 * dir)) & 0xff;
+            const int sc = ((ck >> 8) & 0xff) + ((ck >> 16) & 0xff);
+            const int c1 = dir == 0 ? cc : (dir == 1 ? cc - sc : cc - sc - 1);
+            t.lo[k - 1][c1] = cmin(t.lo[k - 1][c1], t.lo[k][cc] + 1);
+            t.hi[k - 1][c1] = cmax(t.hi[k - 1][c1], t.hi[k][cc] + 1);
+            if (ci > 1) {
+                const int c2 = dir == 0 ? cc : (dir == 1 ? cc - 2 * sc + 1 : cc - 2 * sc - 1);
+                t.lo[k - 2][c2] = cmin(t.lo[k - 2][c2], t.lo[k][cc]);
+                t.hi[k - 2][c2] = cmax(t.hi[k - 2][c2], t.hi[k][cc] + 1);
+            }
+        }
+    return t;
+}
+constexpr int ket_need_nm_max(const KetNeed &t, int k) {
+    int m = 0;
+    for (int c = 0; c < nc(k); ++c) m = cmax(m, t.hi[k][c] - t.lo[k][c] + 1);
+    return m;
+}
+
 template <int LX, int LA, int LB>
 struct GrpCls {
     static_assert(LA >= LB, "canonical order");
@@ -64,9 +99,13 @@ struct GrpCls {
     static constexpr int G_AUTO = cmin(256, pow2ceil(cmax(1, (512 * SLOT * 8 + 200 * 1024 - 1) / (200 * 1024))));
 };
 
-// Tuning hook: group size per class (0 = automatic).
+// Tuning hook: group size per class (0 = automatic); specialisations in lx_tune.h.
 template <int LX, int LA, int LB>
 struct GrpTune { static constexpr int G = 0; };
+
+}  // namespace lx
+#include "lx_tune.h"
+namespace lx {
 
 template <int G>
 __device__ __forceinline__ void group_sync(int group_in_block) {
@@ -100,16 +139,22 @@ __device__ __forceinline__ void build_tables(GrpTables *t, int tid, int nthreads
     }
 }
 
+#ifdef LX_FORCE_RC
+constexpr int GRP_RC = LX_FORCE_RC;
+#else
 constexpr int GRP_RC = 4;  // items a lane keeps decoded in registers at a time
+#endif
 
-template <int LX, int LA, int LB, int MODE, int G, int NTHREADS>
-__global__ void __launch_bounds__(NTHREADS)
+template <int LX, int LA, int LB, int MODE, int G, int NTHREADS, int MINB>
+__global__ void __launch_bounds__(NTHREADS, MINB)
 group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const double *__restrict__ boys_tab,
              double *__restrict__ out, int swapped, DfArgs df) {
     using C = GrpCls<LX, LA, LB>;
     constexpr int L = C::L, E = C::E, NG = C::NG, SLOT = C::SLOT;
     constexpr int GPB = NTHREADS / G;                       // groups (shell-sets) per block
     constexpr int NXC = nc(LX), NA = nc(LA), NB = nc(LB);
+    constexpr KetNeed NEED = ket_need(LX);
+    constexpr int M0 = NEED.lo[0][0];                       // lowest order of [a0|0]^(m) any VRR2 path reads
 
     extern __shared__ double smem[];
     GrpTables *tabs = reinterpret_cast<GrpTables *>(smem + (size_t)GPB * SLOT);
@@ -178,7 +223,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 const double T = g * zc * igz * (PCx * PCx + PCy * PCy + PCz * PCz);
                 // eq. 4 prefactor 2π^{5/2}/(γ ζc sqrt(γ+ζc)) · K_ij · c_k, times F_m(T): one lane per m
                 const double pref = 34.98683665524972497 * Kij * cx * sqrt(igz) / (g * zc);
-                for (int m = lane; m <= L; m += G) W[m * NG] = pref * boys_one(boys_tab, m, T);
+                for (int m = M0 + lane; m <= L; m += G) W[m * NG] = pref * boys_one(boys_tab, m, T);
             } else {
                 PA[0] = PA[1] = PA[2] = WP[0] = WP[1] = WP[2] = WQ[0] = WQ[1] = WQ[2] = 0.0;
             }
@@ -187,7 +232,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             // ---- a3: VRR1 (eq. 3), lanes over the components of shell e, m in registers -----------------------------
             static_for<1, E + 1>([&](auto ie) {
                 constexpr int e = decltype(ie)::value;
-                constexpr int ne = nc(e), nm = L - e + 1;
+                constexpr int ne = nc(e), nm = L - e + 1 - M0;       // orders M0 .. L-e
                 if (on) {
                     for (int ci = lane; ci < ne; ci += G) {
                         const int g0 = off(e) + ci;
@@ -197,26 +242,25 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                         const int g1 = (dn[g0] >> (8 * dir)) & 0xff;
                         const double pa = dir == 0 ? PA[0] : (dir == 1 ? PA[1] : PA[2]);
                         const double wp = dir == 0 ? WP[0] : (dir == 1 ? WP[1] : WP[2]);
-                        double lo1 = W[g1];
+                        // all loads of this component first, then the arithmetic, then the stores (the compiler
+                        // cannot move a shared-memory load above an earlier store on its own)
+                        double v1[nm + 1];
+#pragma unroll
+                        for (int m = 0; m <= nm; ++m) v1[m] = W[(M0 + m) * NG + g1];
                         if (ai > 1) {
                             const int g2 = (dn[g1] >> (8 * dir)) & 0xff;
                             const double c2 = (double)(ai - 1) * o2g;
-                            double lo2 = W[g2];
+                            double v2[nm + 1];
 #pragma unroll
-                            for (int m = 0; m < nm; ++m) {
-                                const double hi1 = W[(m + 1) * NG + g1], hi2 = W[(m + 1) * NG + g2];
-                                W[m * NG + g0] = fma(c2, fma(mrg, hi2, lo2), fma(wp, hi1, pa * lo1));
-                                lo1 = hi1;
-                                lo2 = hi2;
-                            }
+                            for (int m = 0; m <= nm; ++m) v2[m] = W[(M0 + m) * NG + g2];
+#pragma unroll
+                            for (int m = 0; m < nm; ++m) v1[m] = fma(c2, fma(mrg, v2[m + 1], v2[m]), fma(wp, v1[m + 1], pa * v1[m]));
                         } else {
 #pragma unroll
-                            for (int m = 0; m < nm; ++m) {
-                                const double hi1 = W[(m + 1) * NG + g1];
-                                W[m * NG + g0] = fma(wp, hi1, pa * lo1);
-                                lo1 = hi1;
-                            }
+                            for (int m = 0; m < nm; ++m) v1[m] = fma(wp, v1[m + 1], pa * v1[m]);
                         }
+#pragma unroll
+                        for (int m = 0; m < nm; ++m) W[(M0 + m) * NG + g0] = v1[m];
                     }
                 }
                 group_sync<G>(grp);
@@ -232,7 +276,8 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             }
             static_for<1, LX + 1>([&](auto ik) {
                 constexpr int k = decltype(ik)::value;
-                constexpr int nk = nc(k), NAk = C::NAk(k), bk = C::base(k), nm = LX - k + 1;
+                constexpr int nk = nc(k), NAk = C::NAk(k), bk = C::base(k);
+                constexpr int nm = ket_need_nm_max(NEED, k);        // most orders any ket component of this level needs
                 constexpr int NIT = nm * NAk;
                 // source levels k-1 (S1) and k-2 (S2); level 0 is the VRR1 region [m][g]
                 constexpr int o1 = (k == 1) ? 0 : C::boff(k - 1), n1c = nc(k - 1);
@@ -243,7 +288,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 if (on) {
                     for (int r0 = lane; r0 < NIT; r0 += G * GRP_RC) {
                         // decode up to GRP_RC (m, a) items of this lane once; reused for every ket component
-                        int s1[GRP_RC], s1d[GRP_RC][3], s2[GRP_RC], dst[GRP_RC];
+                        int s1[GRP_RC], s1d[GRP_RC][3], s2[GRP_RC], dst[GRP_RC], mq[GRP_RC];
                         double fa[GRP_RC][3];
 #pragma unroll
                         for (int j = 0; j < GRP_RC; ++j) {
@@ -262,6 +307,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                             }
                             s2[j] = m * n2c * NA2 - b2 + ga;
                             dst[j] = ok ? ((k < LX) ? m * nk * NAk + gl : gl) : -1;
+                            mq[j] = ok ? m : 99;
                         }
                         static_for<0, nk>([&](auto icc) {
                             constexpr int cc = decltype(icc)::value;
@@ -271,23 +317,36 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                             constexpr int cy = (ck >> 8) & 0xff, cz = (ck >> 16) & 0xff, sc = cy + cz;
                             constexpr int c1 = dir == 0 ? cc : (dir == 1 ? cc - sc : cc - sc - 1);
                             constexpr int c2 = dir == 0 ? cc : (dir == 1 ? cc - 2 * sc + 1 : cc - 2 * sc - 1);
-                            const double f3 = (double)(ci - 1) * o2z;
+                            constexpr int mlo = NEED.lo[k][cc], nmc = NEED.hi[k][cc] - NEED.lo[k][cc] + 1;
+                            if constexpr (nmc > 0) {
+                                const double f3 = (double)(ci - 1) * o2z;
+                                // item order m' is relative to the first order this ket component needs
+                                const double *S1 = W + o1 + c1 * NA1 + mlo * n1c * NA1;
+                                const double *S2 = W + o2 + c2 * NA2 + mlo * n2c * NA2;
+                                double v[GRP_RC];
+                                bool act[GRP_RC];
 #pragma unroll
-                            for (int j = 0; j < GRP_RC; ++j) {
-                                if (dst[j] >= 0) {
-                                    const double *S1 = W + o1 + c1 * NA1;
-                                    double v = WQ[dir] * S1[s1[j]];
-                                    v = fma(fa[j][dir], S1[s1d[j][dir]], v);
-                                    if constexpr (ci > 1) {
-                                        const double *S2 = W + o2 + c2 * NA2;
-                                        v = fma(f3, fma(mrz, S2[s2[j] + n2c * NA2], S2[s2[j]]), v);
+                                for (int j = 0; j < GRP_RC; ++j) {
+                                    act[j] = mq[j] < nmc;
+                                    if (act[j]) {
+                                        v[j] = WQ[dir] * S1[s1[j]];
+                                        v[j] = fma(fa[j][dir], S1[s1d[j][dir]], v[j]);
+                                        if constexpr (ci > 1) v[j] = fma(f3, fma(mrz, S2[s2[j] + n2c * NA2], S2[s2[j]]), v[j]);
                                     }
-                                    if constexpr (k < LX) {
-                                        W[ot + cc * NAk + dst[j]] = v;
-                                    } else {
-                                        double *t = ACC + cc * C::NA_ACC + dst[j];
-                                        *t = (kt == 0) ? v : *t + v;
+                                }
+                                if constexpr (k < LX) {
+#pragma unroll
+                                    for (int j = 0; j < GRP_RC; ++j)
+                                        if (act[j]) W[ot + cc * NAk + mlo * nk * NAk + dst[j]] = v[j];
+                                } else {
+                                    if (kt != 0) {
+#pragma unroll
+                                        for (int j = 0; j < GRP_RC; ++j)
+                                            if (act[j]) v[j] += ACC[cc * C::NA_ACC + dst[j]];
                                     }
+#pragma unroll
+                                    for (int j = 0; j < GRP_RC; ++j)
+                                        if (act[j]) ACC[cc * C::NA_ACC + dst[j]] = v[j];
                                 }
                             }
                         });
@@ -330,9 +389,12 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                         constexpr int dir = cb >> 24;
                         constexpr int by = (cb >> 8) & 0xff, bz = (cb >> 16) & 0xff, sb = by + bz;
                         constexpr int b1 = dir == 0 ? bj : (dir == 1 ? bj - sb : bj - sb - 1);
+                        double v[GRP_RC];
+#pragma unroll
+                        for (int q = 0; q < GRP_RC; ++q) v[q] = fma(AB[dir], src[s0[q] + b1], src[sd[q][dir] + b1]);
 #pragma unroll
                         for (int q = 0; q < GRP_RC; ++q)
-                            if (dst[q] >= 0) dstb[dst[q] + bj] = fma(AB[dir], src[s0[q] + b1], src[sd[q][dir] + b1]);
+                            if (dst[q] >= 0) dstb[dst[q] + bj] = v[q];
                     });
                 }
             }
@@ -382,39 +444,58 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
     }
 }
 
+// Block shape: how many groups share a block, chosen at compile time to maximise resident warps per SM under the
+// shared-memory limit (227 KB per SM / per block).
+struct BlockShape { int nthreads, gpb, blocks_per_sm; size_t smem; };
+constexpr BlockShape pick_shape(int G, size_t slot_bytes) {
+    const size_t limit = 227 * 1024, tab = sizeof(GrpTables) + 16;
+    BlockShape best{0, 0, 0, 0};
+    int best_warps = -1;
+    for (int cand = 4; cand >= 1; --cand) {
+        // G <= 32: cand = warps per block; G > 32: cand = groups per block
+        const int nthreads = G <= 32 ? cand * 32 : cand * G;
+        if (nthreads > 256 && cand > 1) continue;
+        const int gpb = nthreads / G;
+        const size_t smem = (size_t)gpb * slot_bytes + tab;
+        if (smem > limit) continue;
+        int bps = (int)(limit / (smem + 1024));
+        if (bps > 2048 / nthreads) bps = 2048 / nthreads;
+        if (bps > 32) bps = 32;
+        if (bps < 1) bps = 1;
+        const int warps = bps * nthreads / 32;
+        if (warps > best_warps) { best_warps = warps; best = BlockShape{nthreads, gpb, bps, smem}; }
+    }
+    return best;
+}
+
 template <int LX, int LA, int LB, int MODE>
 cudaError_t group_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                          const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                          cudaStream_t stream) {
     using C = GrpCls<LX, LA, LB>;
+#ifdef LX_FORCE_G   // tuning builds only: one group size for every class that fits
+    constexpr int G = (LX_FORCE_G <= 32 && (size_t)(32 / LX_FORCE_G) * C::SLOT * 8 > 220 * 1024) || (size_t)C::SLOT * 8 > 220 * 1024
+                          ? C::G_AUTO : LX_FORCE_G;
+#else
     constexpr int G = GrpTune<LX, LA, LB>::G > 0 ? GrpTune<LX, LA, LB>::G : C::G_AUTO;
-    // threads per block: 128, or the group size if larger; shrink the block when one block's sets overflow shared memory
-    constexpr size_t slot_bytes = (size_t)C::SLOT * 8;
-    constexpr size_t limit = 227 * 1024 - sizeof(GrpTables) - 64;
-    constexpr int NT0 = G > 128 ? G : 128;
-    constexpr int GPB0 = NT0 / G;
-    constexpr int GPB = (GPB0 * slot_bytes <= limit) ? GPB0 : cmax(1, (int)(limit / slot_bytes));
-    constexpr int NT_raw = GPB * G;
-    constexpr int NT = NT_raw < 32 ? 32 : NT_raw;             // at least one warp
-    constexpr int GPBF = NT / G;
-    constexpr size_t smem = (size_t)GPBF * slot_bytes + sizeof(GrpTables) + 16;
-    static_assert(smem <= 227 * 1024, "class does not fit in shared memory");
-    static_assert(G <= 32 || NT % G == 0, "group/ block mismatch");
+#endif
+    constexpr BlockShape shape = pick_shape(G, (size_t)C::SLOT * 8);
+    static_assert(shape.nthreads > 0, "class does not fit in shared memory");
+    constexpr int NT = shape.nthreads;
     static bool configured = false;
-    auto kern = group_kernel<LX, LA, LB, MODE, G, NT>;
+    // register cap: as many blocks per SM as shared memory allows, but never fewer than 96 registers per thread
+    constexpr int MINB = cmax(1, cmin(shape.blocks_per_sm, 65536 / (NT * 96)));
+    auto kern = group_kernel<LX, LA, LB, MODE, G, NT, MINB>;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shape.smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     if (map.nsets <= 0) return cudaSuccess;
-    int per_sm = (int)((227 * 1024) / (smem + 1024));
-    per_sm = cmax(1, cmin(per_sm, 2048 / NT));
-    per_sm = cmin(per_sm, 16);
-    long long blocks = (map.nsets + GPBF - 1) / GPBF;
-    const long long cap = (long long)num_sms * per_sm;
+    long long blocks = (map.nsets + shape.gpb - 1) / shape.gpb;
+    const long long cap = (long long)num_sms * shape.blocks_per_sm;
     if (blocks > cap) blocks = cap;
-    kern<<<(unsigned)blocks, NT, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+    kern<<<(unsigned)blocks, NT, shape.smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
     return cudaGetLastError();
 }
 

@@ -10,7 +10,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liblx.so")
+_SO = os.environ.get("LX_LIBRARY", os.path.join(_HERE, "liblx.so"))   # LX_LIBRARY: alternative build of liblx
 
 if not os.path.exists(_SO):
     raise ImportError(f"{_SO} not found: build the CUDA library first (python -m paper_2210_03192_b200.build); "
