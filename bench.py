@@ -255,7 +255,7 @@ def main():
         fl_set = SURVEY_FLOPS_PER_SET.get(canon, fl_min)
         t_top = class_ms[i_top] * 1e-3
         achieved = fl_set * nsets / t_top / 1e12
-        roofline = {"bound": "alu", "kernel": f"coop_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
+        roofline = {"bound": "alu", "kernel": f"group_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
                     "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
                     "traffic": None, "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
                     "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
