@@ -138,6 +138,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--npair", type=int, default=1024, help="pairs per class (default = config 2)")
     ap.add_argument("--nx", type=int, default=256, help="aux shells per class (default = config 2)")
+    ap.add_argument("--classes", default="", help="profiling aid: restrict the sweep to e.g. '4,2,1;4,0,0' (default: all 45)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -161,6 +162,8 @@ def main():
 
     # ---- inputs: one full config-2 batch per rank (weak scaling: independent shell-sets, no collective) --------
     classes = gen.CONFIG2_CLASSES
+    if args.classes:
+        classes = [tuple(int(v) for v in c.split(",")) for c in args.classes.split(";")]
     seed = 2 + 1000 * rank
     host, devs = {}, {}
     for c in classes:
@@ -274,7 +277,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": WORKLOAD if (args.npair, args.nx) == (1024, 256) else f"reduced config 2: {args.npair} pairs x {args.nx} aux",
+                "config": {"workload": WORKLOAD if (args.npair, args.nx, args.classes) == (1024, 256, "") else f"reduced config 2: {args.npair} pairs x {args.nx} aux, classes {args.classes or 'all'}",
                            "shell_sets_per_step": nsets * len(classes) * world, "integrals_per_step": ints_per_step * world,
                            "l2": "flushed between timed steps (256 MiB fill, outside the timed interval); each step also writes "
                                  f"{ints_per_step * 8 / 1e9:.1f} GB of output",

@@ -92,12 +92,13 @@ __global__ void pair_data_kernel(DevShells prim, const int32_t *__restrict__ pai
             const double za = prim.zeta[prim.prim_off[a] + i], zb = prim.zeta[prim.prim_off[b] + j];
             const double ca = prim.coef[prim.prim_off[a] + i], cb = prim.coef[prim.prim_off[b] + j];
             const double gam = za + zb, ig = 1.0 / gam;
-            const long long o = ((pd_off ? pd_off[p] : p * (long long)kstride) + ij) * 5;
+            const long long o = ((pd_off ? pd_off[p] : p * (long long)kstride) + ij) * PD_STRIDE;
             pd[o + 0] = gam;
             pd[o + 1] = (za * Ax + zb * Bx) * ig;
             pd[o + 2] = (za * Ay + zb * By) * ig;
             pd[o + 3] = (za * Az + zb * Bz) * ig;
             pd[o + 4] = ca * cb * exp(-za * zb * ig * r2);
+            pd[o + 5] = 0.5 * ig;
         }
     }
 }
@@ -249,7 +250,7 @@ int lx_boys(const double *T, int n, int mmax, double *out, void *stream) {
 size_t lx_eri3_workspace_bytes(int lx_, int la, int lb, int nx, int npair, int kmax_pair) {
     (void)lx_; (void)la; (void)lb; (void)nx;
     if (npair <= 0 || kmax_pair <= 0) return 256;
-    return (size_t)npair * (size_t)kmax_pair * 5 * sizeof(double) + 256;
+    return (size_t)npair * (size_t)kmax_pair * PD_STRIDE * sizeof(double) + 256;
 }
 
 int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim, const int32_t *x_idx,
@@ -263,9 +264,9 @@ int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shel
     if ((rc = check_shells(aux, false)) != LX_OK) return rc;
     if ((rc = check_shells(prim, false)) != LX_OK) return rc;
     if (!x_idx || !pair_idx || !out || !workspace) return LX_EINVAL;
-    // kmax_pair is not passed here: the workspace holds npair*kstride*5 doubles, so derive the stride from its size
+    // kmax_pair is not passed here: the workspace holds npair*kstride*PD_STRIDE doubles, so derive the stride from its size
     const size_t avail = workspace_bytes >= 256 ? workspace_bytes - 256 : 0;
-    const long long kstride_ll = (long long)(avail / ((size_t)npair * 5 * sizeof(double)));
+    const long long kstride_ll = (long long)(avail / ((size_t)npair * PD_STRIDE * sizeof(double)));
     if (kstride_ll < 1) return LX_ENOMEM;
     const int kstride = (int)std::min<long long>(kstride_ll, 1 << 20);
     cudaStream_t st = (cudaStream_t)stream;
@@ -463,7 +464,7 @@ int lx_schedule_create(const lx_shells_t *aux, const lx_shells_t *prim, const do
 int64_t lx_schedule_num_sets(const lx_schedule_t *s) { return s ? s->nsets : 0; }
 int64_t lx_schedule_num_integrals(const lx_schedule_t *s) { return s ? s->nints : 0; }
 size_t lx_df_workspace_bytes(const lx_schedule_t *s) {
-    return s ? (size_t)s->prim_pairs * 5 * sizeof(double) + 256 : 256;
+    return s ? (size_t)s->prim_pairs * PD_STRIDE * sizeof(double) + 256 : 256;
 }
 
 static int df_run(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, int mode, const DfArgs &df,

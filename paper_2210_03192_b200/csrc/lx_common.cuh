@@ -48,8 +48,9 @@ struct SetMap {
     const long long *cum;      // [npair+1] or nullptr
 };
 
-// Primitive-pair data: per primitive pair 5 doubles {γ, Px, Py, Pz, K_ij},
+// Primitive-pair data: per primitive pair PD_STRIDE doubles {γ, Px, Py, Pz, K_ij, 1/(2γ)},
 // K_ij = c_i c_j exp(−ζaζb/γ |AB|²)  (the exponential factor of eq. 4).
+constexpr int PD_STRIDE = 6;
 struct PairData {
     const double *pd;
     const long long *pd_off;  // per-pair offset in primitive pairs, or nullptr → p * kstride

@@ -208,7 +208,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             double PA[3], WP[3], WQ[3], o2g = 0, mrg = 0, o2gz = 0, o2z = 0, mrz = 0;
             if (on) {
                 const int kx = kt / Kab, ij = kt - kx * Kab;
-                const double *q = pdat.pd + (po + ij) * 5;
+                const double *q = pdat.pd + (po + ij) * PD_STRIDE;
                 const double g = q[0], Px = q[1], Py = q[2], Pz = q[3], Kij = q[4];
                 const int xo = aux.prim_off[x] + kx;
                 const double zc = aux.zeta[xo], cx = aux.coef[xo];
