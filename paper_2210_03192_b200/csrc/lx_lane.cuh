@@ -52,12 +52,21 @@ struct LaneHdr {
 
 // The ket pyramid of one bra component for one primitive (a4), all in registers.  P holds level 0 on entry
 // (orders NEED.lo[0][0] .. NEED.hi[0][0] of [a0|0]^(m)); the top level |c| = LX is accumulated into ACC (a5).
-// XLANE: fetch the a − 1_i term from the lane src[i] by shuffle (false when the set has a single bra component).
-template <int LX, bool XLANE>
+// How the a − 1_i term is fetched:
+//   XL_NONE   the set has a single bra component (no such term)
+//   XL_SHFL   from lane src[i] by shuffle
+//   XL_FETCH  by shuffle, except lanes with from_pub set: they read what an earlier helper pass published,
+//             pub[node * NPUB + pubidx[i]]  (pubidx[i] = index of a − 1_i among the published components)
+//   XL_PUB    helper pass: shuffle, and lanes with from_pub set publish (slot pubidx[0]) every value a child node
+//             asks its a − 1_i neighbour for; the top level is only published, not evaluated
+enum { XL_NONE = 0, XL_SHFL = 1, XL_FETCH = 2, XL_PUB = 3 };
+template <int LX, int XL, int NPUB>
 __device__ __forceinline__ void ket_pyramid(double *P, double *ACC, const double (&WQ)[3], const double (&fa)[3],
-                                            double o2z, double mrz, const int (&src)[3], bool on) {
+                                            double o2z, double mrz, const int (&src)[3], bool on, bool from_pub,
+                                            const int (&pubidx)[3], double *pub) {
     constexpr KetNeed NEED = ket_need(LX);
     constexpr KetPyr PYR = ket_pyr(NEED, LX);
+    constexpr int N0 = NEED.hi[0][0] - NEED.lo[0][0] + 1;
     static_for<1, LX + 1>([&](auto ik) {
         constexpr int k = decltype(ik)::value;
         static_for<0, nc(k)>([&](auto icc) {
@@ -72,9 +81,20 @@ __device__ __forceinline__ void ket_pyramid(double *P, double *ACC, const double
             static_for<0, (mhi >= mlo ? mhi - mlo + 1 : 0)>([&](auto im) {
                 constexpr int m = mlo + decltype(im)::value;
                 constexpr int i1 = PYR.off[k - 1][c1] + (m + 1 - NEED.lo[k - 1][c1]);
+                constexpr int node = PYR.off[k][cc] + (m - mlo) - N0;      // number of this node among levels 1..LX
                 const double s1 = P[i1];
+                if constexpr (XL == XL_PUB) {
+                    if (from_pub) pub[node * NPUB + pubidx[0]] = s1;
+                    if constexpr (k == LX) return;
+                }
                 double v = WQ[dir] * s1;
-                if constexpr (XLANE) v = fma(fa[dir], __shfl_sync(0xffffffffu, s1, src[dir]), v);
+                if constexpr (XL == XL_SHFL || XL == XL_PUB) {
+                    v = fma(fa[dir], __shfl_sync(0xffffffffu, s1, src[dir]), v);
+                } else if constexpr (XL == XL_FETCH) {
+                    double nb = __shfl_sync(0xffffffffu, s1, src[dir]);
+                    if (from_pub) nb = pub[node * NPUB + pubidx[dir]];
+                    v = fma(fa[dir], nb, v);
+                }
                 if constexpr (ci > 1) {
                     constexpr int i2 = PYR.off[k - 2][c2] + (m - NEED.lo[k - 2][c2]);
                     v = fma((double)(ci - 1) * o2z, fma(mrz, P[i2 + 1], P[i2]), v);
@@ -89,22 +109,41 @@ __device__ __forceinline__ void ket_pyramid(double *P, double *ACC, const double
     }
 }
 
+// Lane layout of a class.  ES = 0: all NG bra components of a set are lanes of one warp.  ES > 0 ("split"): the
+// components of the shells e >= ES are the MAIN lanes of a set (NGM of them, SPW = 32/NGM sets per warp); the NHC
+// components of the shells e < ES are evaluated first by a HELPER pass of the same warp, lanes = (primitive slice,
+// set, helper component), which publishes the pyramid values of shell ES−1 to shared memory for the main lanes of
+// shell ES.  ES = 2 turns the 35 components of La+Lb = 4 into 31 main lanes (measured: (4|22) 8.3 -> 3.5 ms, (3|22)
+// 4.5 -> 2.2 ms against the shared-memory group kernel).  For La+Lb = 3 the split (2 x 16 main lanes) measured 12-15 %
+// slower than 20 lanes of one set per warp, so it is used from La+Lb = 4 on only.
 template <int LX, int LA, int LB>
 struct LaneCls {
     using C = GrpCls<LX, LA, LB>;
     static constexpr int L = C::L, E = C::E, NG = C::NG;
-    static constexpr bool fits = NG <= 32;
-    static constexpr int SPW = fits ? 32 / NG : 1;          // shell-sets per warp
-    static constexpr int M0 = ket_need(LX).lo[0][0];        // lowest order of [a0|0]^(m) the ket pyramid reads
+    static constexpr int ES = E >= 4 ? 2 : 0;
+    static constexpr int NHC = off(ES);                     // helper components (shells e < ES)
+    static constexpr int NGM = NG - NHC;                    // main components
+    static constexpr bool fits = NGM <= 32 && LA >= ES;
+    static constexpr int SPW = fits ? 32 / NGM : 1;         // shell-sets per warp
+    static constexpr int NSL = ES > 0 ? 32 / (SPW * NHC) : 1;   // primitive slices of the helper pass
+    static constexpr int NPUB = ES > 0 ? nc(ES - 1) : 1;    // published components (shell ES−1)
+    static constexpr KetNeed NEED = ket_need(LX);
+    static constexpr KetPyr PYR = ket_pyr(NEED, LX);
+    static constexpr int M0 = NEED.lo[0][0];                // lowest order of [a0|0]^(m) the ket pyramid reads
+    static constexpr int N0 = NEED.hi[0][0] - NEED.lo[0][0] + 1;
+    static constexpr int NCH = PYR.total - N0;              // pyramid nodes of the levels 1..LX
     static constexpr int NM0 = L + 1 - M0;                  // orders kept per bra component in the VRR1 region
     static constexpr int NPRM = 17;                         // per-primitive record (odd stride: no bank conflicts)
     static constexpr int V1S = NG > 1 ? ((NM0 * NG) | 1) : 0;   // VRR1 region [m − M0][g] of one primitive, odd stride
+    static constexpr int PUBS = ES > 0 ? ((NCH * NPUB) | 1) : 0;   // published values of one primitive
+    static constexpr int PPS = NPRM + V1S + PUBS;           // doubles staged per primitive
     static constexpr int HDR = (int)(sizeof(LaneHdr) / 8);
     static constexpr int NFIN = C::NACC + 2 * C::NH;        // (e0|c) + the two HRR buffers
-    // primitives staged per chunk: as many as fit the warp's share of shared memory (1700 doubles = 13.6 KB, so that
-    // 16 warps are resident per SM), at most 16
-    static constexpr int KB = NG > 1 ? cmax(1, cmin(16, (1700 / SPW - HDR) / (NPRM + V1S))) : 0;
-    static constexpr int SLOT = HDR + cmax(KB * (NPRM + V1S), NFIN);   // doubles of shared memory per set
+    // primitives staged per chunk: as many as fit the warp's share of shared memory (1700 doubles = 13.6 KB for 16
+    // resident warps per SM; 2266 = 18 KB for 12 warps where the published values need the room), at most 16
+    static constexpr int BUDGET = ES > 0 ? 2266 : 1700;
+    static constexpr int KB = NG > 1 ? cmax(1, cmin(16, (cmax(BUDGET, SPW * (HDR + NFIN)) / SPW - HDR) / PPS)) : 0;
+    static constexpr int SLOT = HDR + cmax(KB * PPS, NFIN); // doubles of shared memory per set
 };
 
 // Prefactor record of one primitive triple (phase A → phases B, C, D).
@@ -117,21 +156,22 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
     using C = GrpCls<LX, LA, LB>;
     using LC = LaneCls<LX, LA, LB>;
     constexpr int L = C::L, E = C::E, NG = C::NG, SPW = LC::SPW, SLOT = LC::SLOT;
+    constexpr int ES = LC::ES, NHC = LC::NHC, NGM = LC::NGM, NSL = LC::NSL, NPUB = LC::NPUB;
     constexpr int NXC = nc(LX), NA = nc(LA), NB = nc(LB);
-    constexpr KetNeed NEED = ket_need(LX);
-    constexpr KetPyr PYR = ket_pyr(NEED, LX);
-    constexpr int M0 = LC::M0, NM0 = LC::NM0, NPRM = LC::NPRM, V1S = LC::V1S, KB = LC::KB, HDR = LC::HDR;
-    constexpr int N0 = NEED.hi[0][0] - NEED.lo[0][0] + 1;   // orders of [a0|0]^(m) the pyramid reads
+    constexpr KetPyr PYR = LC::PYR;
+    constexpr int M0 = LC::M0, NM0 = LC::NM0, N0 = LC::N0;
+    constexpr int NPRM = LC::NPRM, V1S = LC::V1S, PUBS = LC::PUBS, KB = LC::KB, HDR = LC::HDR;
+    constexpr int O_V1 = HDR + KB * NPRM, O_PUB = O_V1 + KB * V1S;   // slot layout: header | records | VRR1 | published
     constexpr unsigned FULL = 0xffffffffu;
 
     extern __shared__ double smem[];
     GrpTables *tabs = reinterpret_cast<GrpTables *>(smem + (size_t)NWARPS * SPW * SLOT);
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
-    // lane → (set slot of the warp, bra component); lanes beyond SPW*NG shadow slot 0 / component 0 and never write
-    const bool active = lane < SPW * NG;
-    const int slot = active ? lane / NG : 0;
-    const int g = active ? lane - slot * NG : 0;
+    // main lane → (set slot of the warp, bra component); lanes beyond SPW*NGM shadow slot 0 and never write
+    const bool active = lane < SPW * NGM;
+    const int slot = active ? lane / NGM : 0;
+    const int g = NHC + (active ? lane - slot * NGM : 0);
     double *wbase = smem + (size_t)warp * SPW * SLOT;
     double *myslot = wbase + (size_t)slot * SLOT;
 
@@ -140,14 +180,34 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
     __syncthreads();
     const uint32_t *cart = tabs->cart, *dn = tabs->dn, *up = tabs->up;
 
-    // per-lane constants of the owned bra component
+    // per-lane constants of the owned (main) bra component
     const uint32_t ce_own = cart[g], dn_own = dn[g];
     const int a_own[3] = {(int)(ce_own & 0xff), (int)((ce_own >> 8) & 0xff), (int)((ce_own >> 16) & 0xff)};
     const int e_own = a_own[0] + a_own[1] + a_own[2];
-    int src[3];                                               // lane that owns a − 1_i (self where a_i = 0)
+    const bool fetch_pub = ES > 0 && e_own == ES;             // a − 1_i lives in the helper pass
+    int src[3], pubidx[3];                                    // lane / published slot that owns a − 1_i
 #pragma unroll
-    for (int d = 0; d < 3; ++d) src[d] = active ? slot * NG + (int)((dn_own >> (8 * d)) & 0xff) : lane;
+    for (int d = 0; d < 3; ++d) {
+        const int gd = (int)((dn_own >> (8 * d)) & 0xff);     // cumulative index of a − 1_d (g itself where a_d = 0)
+        src[d] = (active && !fetch_pub) ? slot * NGM + gd - NHC : lane;
+        pubidx[d] = (fetch_pub && gd != g) ? gd - off(ES > 0 ? ES - 1 : 0) : 0;
+    }
     const double fa0[3] = {(double)a_own[0], (double)a_own[1], (double)a_own[2]};
+    // helper lane → (primitive slice, set slot, helper component)
+    const int h_sl = ES > 0 ? lane / (SPW * NHC) : 0;
+    const int h_slot = ES > 0 ? (lane % (SPW * NHC)) / NHC : 0;
+    const int h_g = ES > 0 ? lane % NHC : 0;
+    const bool h_active = ES > 0 && lane < NSL * SPW * NHC;
+    const uint32_t h_ce = cart[h_g], h_dn = dn[h_g];
+    const bool h_pub = ES > 0 && h_active && h_g >= off(ES > 0 ? ES - 1 : 0);
+    int h_src[3], h_pubidx[3];
+    double h_fa0[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        h_src[d] = h_active ? lane - h_g + (int)((h_dn >> (8 * d)) & 0xff) : lane;
+        h_pubidx[d] = h_pub ? h_g - off(ES > 0 ? ES - 1 : 0) : 0;
+        h_fa0[d] = (double)((h_ce >> (8 * d)) & 0xff);
+    }
 
     const long long wstride = (long long)gridDim.x * NWARPS * SPW;
     for (long long sbase = ((long long)blockIdx.x * NWARPS + warp) * SPW; sbase < map.nsets; sbase += wstride) {
@@ -224,11 +284,11 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
 #pragma unroll
                 for (int i = 0; i < N0; ++i) P[PYR.off[0][0] + i] = pref * F[M0 + i];
                 const double fa[3] = {0.0, 0.0, 0.0};
-                ket_pyramid<LX, false>(P, ACC, WQ, fa, o2z, mrz, src, on);
+                ket_pyramid<LX, XL_NONE, 1>(P, ACC, WQ, fa, o2z, mrz, src, on, false, pubidx, nullptr);
             }
         } else {
             LaneHdr *hdr = reinterpret_cast<LaneHdr *>(myslot);
-            if (active && g == 0) {
+            if (active && g == NHC) {
                 hdr->A[0] = Ax; hdr->A[1] = Ay; hdr->A[2] = Az;
                 hdr->C[0] = Cx; hdr->C[1] = Cy; hdr->C[2] = Cz;
                 hdr->po = po; hdr->xo0 = xo0; hdr->Kab = Kab; hdr->K = K;
@@ -269,7 +329,7 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                     double *sl = wbase + (size_t)s * SLOT;
                     if (k0 + kk < reinterpret_cast<const LaneHdr *>(sl)->K) {
                         const double *pr = sl + HDR + kk * NPRM;
-                        sl[HDR + KB * NPRM + kk * V1S + mi * NG] = pr[PR_PREF] * boys_one(boys_tab, M0 + mi, pr[PR_T]);
+                        sl[O_V1 + kk * V1S + mi * NG] = pr[PR_PREF] * boys_one(boys_tab, M0 + mi, pr[PR_T]);
                     }
                 }
                 __syncwarp();
@@ -282,7 +342,7 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                         double *sl = wbase + (size_t)s * SLOT;
                         if (k0 + kk < reinterpret_cast<const LaneHdr *>(sl)->K) {
                             const double *pr = sl + HDR + kk * NPRM;
-                            double *Wk = sl + HDR + KB * NPRM + kk * V1S;
+                            double *Wk = sl + O_V1 + kk * V1S;
                             const int g0 = off(e) + ci;
                             const uint32_t ce = cart[g0];
                             const int dir = ce >> 24;
@@ -310,18 +370,39 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                     }
                     __syncwarp();
                 });
+                // ---- phase D0 (a4): helper pass, shells e < ES; lanes over (primitive slice, set, component) -------------------
+                if constexpr (ES > 0) {
+                    double *hsl = wbase + (size_t)h_slot * SLOT;
+                    const int hK = reinterpret_cast<const LaneHdr *>(hsl)->K;
+                    for (int kb = 0; kb < KBc; kb += NSL) {   // warp-uniform trip count
+                        const int kk = min(kb + h_sl, KB - 1);
+                        const bool hon = h_active && kb + h_sl < KBc && k0 + kb + h_sl < hK;
+                        const double *pr = hsl + HDR + kk * NPRM;
+                        const double *Wk = hsl + O_V1 + kk * V1S;
+                        double P[PYR.total];
+#pragma unroll
+                        for (int i = 0; i < N0; ++i) P[PYR.off[0][0] + i] = Wk[i * NG + h_g];
+                        const double WQ[3] = {pr[PR_WQ], pr[PR_WQ + 1], pr[PR_WQ + 2]};
+                        const double o2gz = pr[PR_O2GZ], o2z = pr[PR_O2Z], mrz = pr[PR_MRZ];
+                        const double fa[3] = {h_fa0[0] * o2gz, h_fa0[1] * o2gz, h_fa0[2] * o2gz};
+                        ket_pyramid<LX, XL_PUB, NPUB>(P, ACC, WQ, fa, o2z, mrz, h_src, false, h_pub && hon, h_pubidx,
+                                                      hsl + O_PUB + kk * PUBS);
+                    }
+                    __syncwarp();
+                }
                 // ---- phase D (a4/a5): VRR2 in registers, one primitive after the other; no synchronisation inside ----------
                 for (int kk = 0; kk < KBc; ++kk) {
                     const bool on = k0 + kk < K;
                     const double *pr = myslot + HDR + kk * NPRM;
-                    const double *Wk = myslot + HDR + KB * NPRM + kk * V1S;
+                    const double *Wk = myslot + O_V1 + kk * V1S;
                     double P[PYR.total];
 #pragma unroll
                     for (int i = 0; i < N0; ++i) P[PYR.off[0][0] + i] = Wk[i * NG + g];
                     const double WQ[3] = {pr[PR_WQ], pr[PR_WQ + 1], pr[PR_WQ + 2]};
                     const double o2gz = pr[PR_O2GZ], o2z = pr[PR_O2Z], mrz = pr[PR_MRZ];
                     const double fa[3] = {fa0[0] * o2gz, fa0[1] * o2gz, fa0[2] * o2gz};
-                    ket_pyramid<LX, true>(P, ACC, WQ, fa, o2z, mrz, src, on);
+                    ket_pyramid<LX, (ES > 0 ? XL_FETCH : XL_SHFL), NPUB>(P, ACC, WQ, fa, o2z, mrz, src, on, fetch_pub, pubidx,
+                                                                       myslot + O_PUB + kk * PUBS);
                 }
                 __syncwarp();
             }
@@ -342,7 +423,7 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
             double *SW = SA + C::NACC;
             double ABs[3];
 #pragma unroll
-            for (int d = 0; d < 3; ++d) ABs[d] = __shfl_sync(FULL, AB[d], s * NG);
+            for (int d = 0; d < 3; ++d) ABs[d] = __shfl_sync(FULL, AB[d], s * NGM);
             static_for<1, LB + 1>([&](auto ij_) {
                 constexpr int j = decltype(ij_)::value;
                 constexpr int nbj = nc(j), NAj = C::NAH(j), nb1 = nc(j - 1), NA1 = C::NAH(j - 1);
@@ -393,8 +474,8 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                     }
                 }
             } else {
-                const int as = __shfl_sync(FULL, a, s * NG), bs = __shfl_sync(FULL, b, s * NG),
-                          xs_ = __shfl_sync(FULL, x, s * NG);
+                const int as = __shfl_sync(FULL, a, s * NGM), bs = __shfl_sync(FULL, b, s * NGM),
+                          xs_ = __shfl_sync(FULL, x, s * NGM);
                 if constexpr (MODE == 1) {
                     // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
                     const double *Dab = df.D + (size_t)prim.bf_off[as] * df.ld + prim.bf_off[bs];
