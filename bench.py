@@ -254,15 +254,20 @@ def main():
         i_top = int(np.argmax(class_ms))
         c_top = classes[i_top]
         canon = (c_top[0], max(c_top[1:]), min(c_top[1:]))
-        fl_min = costmodel.flops_per_set(*c_top, 9)
-        fl_set = SURVEY_FLOPS_PER_SET.get(canon, fl_min)
+        # algorithmic flops per shell-set: the component-level DAG count of costmodel.py; SURVEY.md
+        # §8(d) quotes a larger figure for some classes (it over-counts: ncu's executed DFMA/DMUL/DADD count matches
+        # the cost model, profiles/r01_ncu_lane_4_2_2.md) and is reported next to it
+        fl_set = costmodel.flops_per_set(*c_top, 9)
+        fl_survey = SURVEY_FLOPS_PER_SET.get(canon)
         t_top = class_ms[i_top] * 1e-3
         achieved = fl_set * nsets / t_top / 1e12
-        roofline = {"bound": "alu", "kernel": f"group_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
+        roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family(*canon)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
                     "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
                     "traffic": None, "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
                     "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
-                    "flops_per_set_min_model": fl_min, "kernel_ms": class_ms[i_top],
+                    "flops_per_set_survey": fl_survey,
+                    "frac_with_survey_flops": (fl_survey * nsets / t_top / 1e12 / FP64_NOMINAL_TFLOPS) if fl_survey else None,
+                    "kernel_ms": class_ms[i_top],
                     "share_of_step": float(class_ms[i_top] / class_ms.sum()),
                     "hbm_write_gbs": nint_set(c_top) * 8 * nsets / t_top / 1e9}
         cpu = None

@@ -137,6 +137,10 @@ int lx_boys(const double *T, int n, int mmax, double *out, void *stream);
  * 5 timed launches.  This is the measured denominator of the FP64-pipe roofline; synchronises. */
 int lx_fp64_probe(int iters, double *tflops_host);
 
+/* Which kernel template serves a class: "lane" (register-resident, lx_lane.cuh) or "group" (shared-memory,
+ * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only. */
+const char *lx_kernel_family(int lx, int la, int lb);
+
 /* Number of kernel launches the library has issued since lx_init (for the bench's `gpu_launches` claim). */
 int64_t lx_launch_count(void);
 

@@ -12,6 +12,7 @@
 
 #include "lx_common.cuh"
 #include "lx_dispatch.h"
+#include "lx_lane.cuh"
 
 namespace lx {
 
@@ -160,6 +161,11 @@ using namespace lx;
 extern "C" {
 
 const char *lx_version(void) { return "lx3 0.1 sm_100a (coop kernels, Lx<=6, La,Lb<=4)"; }
+
+const char *lx_kernel_family(int lx_, int la, int lb) {
+    if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
+    return lane_fits(std::max(la, lb), std::min(la, lb)) ? "lane" : "group";
+}
 
 const char *lx_strerror(int status) {
     switch (status) {

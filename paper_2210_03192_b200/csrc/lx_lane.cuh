@@ -116,14 +116,20 @@ __device__ __forceinline__ void ket_pyramid(double *P, double *ACC, const double
 // shell ES.  ES = 2 turns the 35 components of La+Lb = 4 into 31 main lanes (measured: (4|22) 8.3 -> 3.5 ms, (3|22)
 // 4.5 -> 2.2 ms against the shared-memory group kernel).  For La+Lb = 3 the split (2 x 16 main lanes) measured 12-15 %
 // slower than 20 lanes of one set per warp, so it is used from La+Lb = 4 on only.
+__host__ __device__ constexpr int lane_es(int E) { return E >= 4 ? 2 : 0; }
+// does the class (La >= Lb) run on the lane kernel?  (otherwise: the shared-memory group kernel)
+__host__ __device__ constexpr bool lane_fits(int LA, int LB) {
+    return off(LA + LB + 1) - off(lane_es(LA + LB)) <= 32 && LA >= lane_es(LA + LB);
+}
+
 template <int LX, int LA, int LB>
 struct LaneCls {
     using C = GrpCls<LX, LA, LB>;
     static constexpr int L = C::L, E = C::E, NG = C::NG;
-    static constexpr int ES = E >= 4 ? 2 : 0;
+    static constexpr int ES = lane_es(E);
     static constexpr int NHC = off(ES);                     // helper components (shells e < ES)
     static constexpr int NGM = NG - NHC;                    // main components
-    static constexpr bool fits = NGM <= 32 && LA >= ES;
+    static constexpr bool fits = lane_fits(LA, LB);
     static constexpr int SPW = fits ? 32 / NGM : 1;         // shell-sets per warp
     static constexpr int NSL = ES > 0 ? 32 / (SPW * NHC) : 1;   // primitive slices of the helper pass
     static constexpr int NPUB = ES > 0 ? nc(ES - 1) : 1;    // published components (shell ES−1)

@@ -22,7 +22,7 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
-           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe"]
+           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family"]
 
 
 class lx_shells_t(C.Structure):
@@ -32,6 +32,8 @@ class lx_shells_t(C.Structure):
 
 _lib.lx_strerror.restype = C.c_char_p
 _lib.lx_version.restype = C.c_char_p
+_lib.lx_kernel_family.restype = C.c_char_p
+_lib.lx_kernel_family.argtypes = [C.c_int] * 3
 _lib.lx_eri3_workspace_bytes.restype = C.c_size_t
 _lib.lx_df_workspace_bytes.restype = C.c_size_t
 _lib.lx_df_workspace_bytes.argtypes = [C.c_void_p]
@@ -72,6 +74,10 @@ def ncart(l):
 
 def lx_version():
     return _lib.lx_version().decode()
+
+
+def lx_kernel_family(lx, la, lb):
+    return _lib.lx_kernel_family(lx, la, lb).decode()
 
 
 def lx_strerror(status):
