@@ -1,7 +1,7 @@
 // lx_inst.cu — instantiates the class kernels for one aux angular momentum (INST_LX) and one digestion mode
 // (INST_MODE: 0 store, 1 γ, 2 J).  Compiled once per (INST_LX, INST_MODE); no code generator: every class is a
 // template instantiation.
-#include "lx_lane.cuh"
+#include "lx_chain.cuh"
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
@@ -16,7 +16,9 @@ template <int LX, int LA, int LB, int MODE>
 static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                                 const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                                 cudaStream_t stream) {
-    if constexpr (LaneCls<LX, LA, LB>::fits)
+    if constexpr (ChainCls<LX, LA, LB>::fits)
+        return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else if constexpr (LaneCls<LX, LA, LB>::fits)
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
