@@ -12,7 +12,7 @@
 
 #include "lx_common.cuh"
 #include "lx_dispatch.h"
-#include "lx_chain.cuh"
+#include "lx_team.cuh"
 
 namespace lx {
 
@@ -164,7 +164,12 @@ const char *lx_version(void) { return "lx3 0.1 sm_100a (coop kernels, Lx<=6, La,
 
 const char *lx_kernel_family(int lx_, int la, int lb) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
-    if (chain_fits(lx_, std::max(la, lb), std::min(la, lb))) return "chain";
+    {
+        const int ca = std::max(la, lb), cb = std::min(la, lb);
+        const int tw = (ca + cb <= 4 && lx_ <= 4) ? team_size(lx_, ca, cb, 56) : 0;
+        if (tw > 0 && (ca + cb <= 2 || tw <= 2)) return "team";
+        if (chain_fits(lx_, ca, cb)) return "chain";
+    }
     return lane_fits(std::max(la, lb), std::min(la, lb)) ? "lane" : "group";
 }
 

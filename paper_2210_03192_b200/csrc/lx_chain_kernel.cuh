@@ -1,0 +1,247 @@
+// lx_chain_kernel.cuh — the warp-specialised chain kernel (design and algebra: lx_chain.cuh; shared per-primitive
+// arithmetic, target drop and epilogue: lx_team.cuh).
+#pragma once
+#include "lx_team.cuh"
+
+namespace lx {
+
+template <int LX, int LA, int LB, int MODE, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB)
+chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const double *__restrict__ boys_tab,
+             double *__restrict__ out, int swapped, DfArgs df) {
+    using CC = ChainCls<LX, LA, LB>;
+    constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NXC = CC::NXC, NA = CC::NA, NB = CC::NB, NAB = CC::NAB;
+    constexpr int SLOTN = CC::SLOTN;
+    constexpr ChainTargets T = CC::T;
+    constexpr ChainPlan P = CC::P;
+    constexpr unsigned FULL = 0xffffffffu;
+
+    extern __shared__ double smem[];
+    double *TC = smem;                                       // [set][c * NAB + ·]: (e0|c), then the finished shell-set
+    double *ZB = TC + (size_t)32 * SLOTN;                    // ring of start-vector buffers
+    double *hd = ZB + (size_t)CC::ZBD;                 // header doubles [9][32]: A, C, AB
+    long long *hpo = reinterpret_cast<long long *>(hd + 9 * 32);
+    int *hi = reinterpret_cast<int *>(hpo + 32);             // [6][32]: xo0, Kab, K, a, b, x
+    int *s_kmax = hi + 6 * 32;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long nbatch = (map.nsets + 31) / 32;
+
+    for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
+        // ---- set of each lane (warp 0 decodes, everybody reads the header) ---------------------------------------------
+        if (warp == 0) {
+            const long long sid = batch * 32 + lane;
+            const bool live = sid < map.nsets;
+            int p = 0, xs = 0;
+            if (live) {
+                if (map.cum == nullptr) {
+                    p = (int)(sid / map.nx);
+                    xs = (int)(sid - (long long)p * map.nx);
+                } else {
+                    int lo = 0, hi_ = map.npair;             // largest p with cum[p] <= sid
+                    while (hi_ - lo > 1) {
+                        const int mid = (lo + hi_) >> 1;
+                        if (map.cum[mid] <= sid) lo = mid; else hi_ = mid;
+                    }
+                    p = lo;
+                    xs = (int)(sid - map.cum[p]);
+                }
+            }
+            const int a = map.pair_list[2 * p + swapped], b = map.pair_list[2 * p + 1 - swapped];
+            const int x = map.x_list[xs];
+            const int Kab = prim.K[a] * prim.K[b];
+            const int K = live ? Kab * aux.K[x] : 0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const double Ad = prim.center[3 * a + d];
+                hd[d * 32 + lane] = Ad;
+                hd[(3 + d) * 32 + lane] = aux.center[3 * x + d];
+                hd[(6 + d) * 32 + lane] = Ad - prim.center[3 * b + d];
+            }
+            hpo[lane] = pdat.pd_off ? pdat.pd_off[p] : (long long)p * pdat.kstride;
+            hi[0 * 32 + lane] = aux.prim_off[x];
+            hi[1 * 32 + lane] = Kab;
+            hi[2 * 32 + lane] = K;
+            hi[3 * 32 + lane] = a;
+            hi[4 * 32 + lane] = b;
+            hi[5 * 32 + lane] = x;
+            const int km = __reduce_max_sync(FULL, K);
+            if (lane == 0) *s_kmax = km;
+        }
+        __syncthreads();
+        const int kmax = *s_kmax;
+
+        // ---- passes over the primitive loop --------------------------------------------------------------------------------
+        static_for<0, P.npass>([&](auto ipass) {
+            constexpr int ip = decltype(ipass)::value;
+            constexpr int T0 = P.t0[ip], NC = P.t1[ip] - P.t0[ip], PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
+            constexpr int NPROD = P.nprod[ip], NBUF = NPROD + 1, ZREC = chain_zrec(NLV, NG);
+            constexpr int BCOUNT = (NC + 1) * 32;            // threads on a full[] / empty[] barrier
+            double acc[NACC];
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+
+            if (warp >= NC && warp < NC + NPROD) {
+                // ================= producer: primitives q = j, j + NPROD, ... =================================================
+                const int j = warp - NC;
+                const double Ax = hd[0 * 32 + lane], Ay = hd[1 * 32 + lane], Az = hd[2 * 32 + lane];
+                const double Cx = hd[3 * 32 + lane], Cy = hd[4 * 32 + lane], Cz = hd[5 * 32 + lane];
+                const long long po = hpo[lane];
+                const int xo0 = hi[0 * 32 + lane], Kab = hi[1 * 32 + lane], K = hi[2 * 32 + lane];
+                for (int q = j; q < kmax; q += NPROD) {
+                    const int bsel = q % NBUF;
+                    if (q >= NBUF) named_sync(1 + NBUF + bsel, BCOUNT);      // consumers are done with this buffer
+                    double *zb = ZB + (size_t)bsel * ZREC;
+                    const bool on = q < K;
+                    const int qq = on ? q : 0;
+                    const int kx = qq / Kab, ij = qq - kx * Kab;
+                    const double zc = aux.zeta[xo0 + kx], cxc = on ? aux.coef[xo0 + kx] : 0.0;
+                    const double *pq = pdat.pd + (po + ij) * PD_STRIDE;
+                    const double gm = __ldg(pq), Px = __ldg(pq + 1), Py = __ldg(pq + 2), Pz = __ldg(pq + 3),
+                                 Kij = __ldg(pq + 4), o2g = __ldg(pq + 5);
+                    const double PCx = Px - Cx, PCy = Py - Cy, PCz = Pz - Cz;
+                    const double o2z = 0.5 / zc;
+                    const double sq = rsqrt(gm + zc);         // (γ+ζc)^{-1/2}
+                    const double igz = sq * sq;
+                    const double mrg = -zc * igz;             // −ρ/γ
+                    const double mrz = -gm * igz;             // −ρ/ζc
+                    const double PA[3] = {Px - Ax, Py - Ay, Pz - Az};
+                    const double WP[3] = {mrg * PCx, mrg * PCy, mrg * PCz};
+                    const double Tt = gm * zc * igz * (PCx * PCx + PCy * PCy + PCz * PCz);
+                    // eq. 4: 2π^{5/2}/(γ ζc sqrt(γ+ζc)) K_ij c_k = 8π^{5/2} (1/2γ)(1/2ζc)(γ+ζc)^{-1/2} K_ij c_k
+                    const double pref = 139.94734662099889988 * Kij * cxc * o2g * o2z * sq;
+                    const double g2 = gm + gm;
+                    const double cs = 0.5 * igz;              // 1/(2(γ+ζc))
+                    double *rec = zb + (size_t)NLV * NG * 32;
+                    rec[0 * 32 + lane] = g2 * PCx;
+                    rec[1 * 32 + lane] = g2 * PCy;
+                    rec[2 * 32 + lane] = g2 * PCz;
+                    // Boys orders LX − 2p .. LX − p + E for the levels of this pass: one table evaluation at the top
+                    constexpr int MLO = LX - 2 * (PLO + NLV - 1), MHI = LX - PLO + E;
+                    double F[MHI - MLO + 1];
+                    if (Tt < (double)BOYS_TMAX) {
+                        F[MHI - MLO] = boys_one(boys_tab, MHI, Tt);
+                        if constexpr (MHI > MLO) {
+                            const double eT = exp(-Tt), T2 = Tt + Tt;
+#pragma unroll
+                            for (int m = MHI; m > MLO; --m) F[m - 1 - MLO] = fma(T2, F[m - MLO], eT) * (1.0 / (double)(2 * m - 1));
+                        }
+                    } else {
+                        double f = 0.5 * sqrt(3.14159265358979323846 / Tt);
+                        const double h = 0.5 / Tt;
+#pragma unroll
+                        for (int m = 0; m <= MHI; ++m) {
+                            if (m >= MLO) F[m - MLO] = f;
+                            f *= (double)(2 * m + 1) * h;
+                        }
+                    }
+                    static_for<0, NLV>([&](auto ilv) {
+                        constexpr int lv = decltype(ilv)::value, p = PLO + lv, k = LX - 2 * p;
+                        // deferred scalar of the level: (1/(2(γ+ζc)))^k (1/(2ζc))^p
+                        double ck = 1.0;
+#pragma unroll
+                        for (int i = 0; i < k; ++i) ck *= cs;
+#pragma unroll
+                        for (int i = 0; i < p; ++i) ck *= o2z;
+                        rec[(3 + lv) * 32 + lane] = ck;
+                        // a3: VRR1 (eq. 3) on W^(m) = pref Σ_s C(p,s) (−ρ/ζc)^s F_{k+m+s}, m = 0..E
+                        constexpr int NV = chain_nv1(E);
+                        double V[NV];
+                        static_for<0, E + 1>([&](auto im) {
+                            constexpr int m = decltype(im)::value;
+                            double w = F[k + m + p - MLO];
+                            static_for<0, p>([&](auto is) {
+                                constexpr int s = p - 1 - decltype(is)::value;     // Horner in (−ρ/ζc)
+                                w = fma(w, mrz, (double)ibinom(p, s) * F[k + m + s - MLO]);
+                            });
+                            V[m] = pref * w;
+                        });
+                        static_for<1, E + 1>([&](auto ie) {
+                            constexpr int e = decltype(ie)::value;
+                            static_for<0, nc(e)>([&](auto ici) {
+                                constexpr int ci = decltype(ici)::value, g = off(e) + ci;
+                                constexpr int dir = (int)(cart_entry(g) >> 24), ai = cart_pow(g, dir);
+                                constexpr int g1 = cart_dn(g, dir), c1 = g1 - off(e - 1);
+                                static_for<0, E - e + 1>([&](auto im) {
+                                    constexpr int m = decltype(im)::value;
+                                    constexpr int i1 = v1_off(E, e - 1) + m * nc(e - 1) + c1;
+                                    double v = fma(WP[dir], V[i1 + nc(e - 1)], PA[dir] * V[i1]);
+                                    if constexpr (ai > 1) {
+                                        constexpr int c2 = cart_dn(g1, dir) - off(e - 2);
+                                        constexpr int i2 = v1_off(E, e - 2) + m * nc(e - 2) + c2;
+                                        v = fma((double)(ai - 1) * o2g, fma(mrg, V[i2 + nc(e - 2)], V[i2]), v);
+                                    }
+                                    V[v1_off(E, e) + m * nc(e) + ci] = v;
+                                });
+                            });
+                        });
+                        // start vector u[a] = Y_p[a] / a!
+                        static_for<0, NG>([&](auto ig) {
+                            constexpr int g = decltype(ig)::value, e = cart_shell(g);
+                            constexpr double inv = 1.0 / (double)cart_fact(g);
+                            zb[((size_t)lv * NG + g) * 32 + lane] = V[v1_off(E, e) + (g - off(e))] * inv;
+                        });
+                    });
+                    __threadfence_block();
+                    named_arrive(1 + bsel, BCOUNT);           // full[bsel]
+                }
+            } else if (warp < NC) {
+                // ================= consumer: target T0 + warp ====================================================================
+                for (int q = 0; q < kmax; ++q) {
+                    const int bsel = q % NBUF;
+                    named_sync(1 + bsel, BCOUNT);             // full[bsel]
+                    const double *zb = ZB + (size_t)bsel * ZREC;
+                    const double *rec = zb + (size_t)NLV * NG * 32;
+                    const double rx = rec[0 * 32 + lane], ry = rec[1 * 32 + lane], rz = rec[2 * 32 + lane];
+                    static_for<0, NC>([&](auto iw) {
+                        constexpr int w = decltype(iw)::value, tg = T.g[T0 + w], lv = T.p[T0 + w] - PLO;
+                        if (warp == w) {
+                            const double ck = rec[(3 + lv) * 32 + lane];
+                            chain_apply<LA, E, cart_pow(tg, 0), cart_pow(tg, 1), cart_pow(tg, 2)>(zb + (size_t)lv * NG * 32, lane, rx, ry, rz, ck, acc);
+                        }
+                    });
+                    if (q + NBUF < kmax) named_arrive(1 + NBUF + bsel, BCOUNT);   // empty[bsel]
+                }
+            }
+            __syncthreads();
+            // ---- drop the contracted targets: level 0 into its Cartesian slot of TC, higher levels into the staging area
+            // (which aliases the ring: all targets of the levels p >= 1 belong to the last pass, whose ring is idle now)
+            static_for<0, NC>([&](auto iw) {
+                constexpr int w = decltype(iw)::value;
+                static_assert(T0 + w < NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
+                if (warp == w) target_drop<LX, LA, LB, T0 + w>(acc, TC, ZB, lane);
+            });
+            __syncthreads();
+        });
+        chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, warp, lane, batch, map, aux, prim, out, swapped, df);
+    }
+}
+
+template <int LX, int LA, int LB, int MODE>
+cudaError_t chain_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
+                         const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
+                         cudaStream_t stream) {
+    using CC = ChainCls<LX, LA, LB>;
+    constexpr int NW = CC::NW;
+    constexpr size_t smem = CC::smem;
+    // resident blocks per SM: shared memory, and registers (a consumer keeps NG + NACC doubles live)
+    constexpr int by_smem = (int)((227 * 1024) / (smem + 1024));
+    constexpr int regs = CC::E <= 2 ? 80 : (CC::E == 3 ? 128 : 168);
+    constexpr int by_regs = 65536 / (NW * 32 * regs);
+    constexpr int BPS = cmax(1, cmin(cmin(by_smem, by_regs), 8));
+    auto kern = chain_kernel<LX, LA, LB, MODE, NW, BPS>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    if (map.nsets <= 0) return cudaSuccess;
+    long long blocks = (map.nsets + 31) / 32;
+    const long long cap = (long long)num_sms * BPS;
+    if (blocks > cap) blocks = cap;
+    kern<<<(unsigned)blocks, NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+    return cudaGetLastError();
+}
+
+}  // namespace lx

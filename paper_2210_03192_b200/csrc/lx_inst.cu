@@ -1,7 +1,10 @@
 // lx_inst.cu — instantiates the class kernels for one aux angular momentum (INST_LX) and one digestion mode
 // (INST_MODE: 0 store, 1 γ, 2 J).  Compiled once per (INST_LX, INST_MODE); no code generator: every class is a
 // template instantiation.
-#include "lx_chain.cuh"
+#include <cstdlib>
+#include <cstring>
+
+#include "lx_chain_kernel.cuh"
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
@@ -10,15 +13,39 @@
 
 namespace lx {
 
-// kernel family per class: register-resident lane kernel where the bra components of a set fit one warp
-// (La+Lb <= 3), shared-memory group kernel otherwise
+// kernel family per class: team kernel where the chain targets of a warp fit its registers,
+// warp-specialised chain kernel for the other classes with La+Lb <= 4 and Lx <= 4, lane / group kernels beyond.
+// LX_FAMILY=team|chain|lane in the environment overrides the choice where the named family exists (tuning aid).
+#ifndef LX_TEAM_BUDGET
+#define LX_TEAM_BUDGET 56
+#endif
+static int family_override() {
+    static int v = -1;
+    if (v < 0) {
+        const char *e = std::getenv("LX_FAMILY");
+        v = !e ? 0 : (!std::strcmp(e, "team") ? 1 : (!std::strcmp(e, "chain") ? 2 : (!std::strcmp(e, "lane") ? 3 : 0)));
+    }
+    return v;
+}
+
 template <int LX, int LA, int LB, int MODE>
 static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                                 const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                                 cudaStream_t stream) {
-    if constexpr (ChainCls<LX, LA, LB>::fits)
-        return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
-    else if constexpr (LaneCls<LX, LA, LB>::fits)
+    constexpr bool small = LA + LB <= 4 && LX <= 4;
+    constexpr int TW = small ? team_size(LX, LA, LB, LX_TEAM_BUDGET) : 0;
+    // measured (config 2, B200): the team kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets
+    constexpr bool has_team = TW > 0 && (LA + LB <= 2 || TW <= 2), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
+    const int ov = family_override();
+    if constexpr (has_team) {
+        if (ov == 0 || ov == 1 || (ov == 2 && !has_chain) || (ov == 3 && !has_lane))
+            return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    }
+    if constexpr (has_chain) {
+        if (ov != 3 || !has_lane)
+            return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    }
+    if constexpr (has_lane)
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
