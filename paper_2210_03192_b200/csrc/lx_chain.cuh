@@ -112,7 +112,7 @@ constexpr ChainPlan chain_plan(int LX, int LA, int LB) {
         int np = (prod + cons - 1) / cons;
         np = cmax(1, cmin(np, cmin(6, nwmax - (P.t1[i] - P.t0[i]))));
         // the ring shares 227 KB with the (e0|c) region of the 32 sets and the header
-        const int room = (227 * 1024) / 8 - 32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) - 520;
+        const int room = (227 * 1024) / 8 - 32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) - 520 - 256;
         while (np > 1 && (np + 1) * chain_zrec(nlev, NG) > room) --np;
         P.nprod[i] = np;
         P.nw = cmax(P.nw, P.t1[i] - P.t0[i] + np);
@@ -133,7 +133,7 @@ struct ChainCls {
     static constexpr int NUB = (T.n - NXC) * NACC * 32;       // staging of the contracted targets of the levels p >= 1
     static constexpr int ZBD = cmax(P.ring, NUB);             // the staging area aliases the ring
     static constexpr int HDRD = 9 * 32 + 32 + 6 * 16;         // header: 9 doubles + 1 int64 + 6 ints per set, in doubles
-    static constexpr size_t smem = ((size_t)32 * SLOTN + (size_t)ZBD + HDRD + 4) * 8;
+    static constexpr size_t smem = ((size_t)32 * SLOTN + (size_t)ZBD + HDRD + 4) * 8 + 2048;   // + partner table
     static constexpr bool fits = E <= 4 && LX <= 4 && P.ok && smem <= 227 * 1024 && NW <= 32;
 };
 __host__ __device__ constexpr bool chain_fits(int LX, int LA, int LB) {
@@ -143,7 +143,7 @@ __host__ __device__ constexpr bool chain_fits(int LX, int LA, int LB) {
     int NT = 0;
     for (int p = 0; 2 * p <= LX; ++p) NT += nc(LX - 2 * p);
     const int nub = (NT - nc(LX)) * NACC * 32;
-    const size_t smem = ((size_t)32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) + (size_t)cmax(P.ring, nub) + 9 * 32 + 32 + 6 * 16 + 4) * 8;
+    const size_t smem = ((size_t)32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) + (size_t)cmax(P.ring, nub) + 9 * 32 + 32 + 6 * 16 + 4) * 8 + 2048;
     return P.ok && smem <= 227 * 1024 && P.nw <= 32;
 }
 

@@ -23,6 +23,8 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
     long long *hpo = reinterpret_cast<long long *>(hd + 9 * 32);
     int *hi = reinterpret_cast<int *>(hpo + 32);             // [6][32]: xo0, Kab, K, a, b, x
     int *s_kmax = hi + 6 * 32;
+    PartnerTab *pt = reinterpret_cast<PartnerTab *>(hd + CC::HDRD + 4);
+    if (threadIdx.x == 0) partner_tab_build<LX>(pt);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long nbatch = (map.nsets + 31) / 32;
@@ -206,14 +208,11 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             __syncthreads();
             // ---- drop the contracted targets: level 0 into its Cartesian slot of TC, higher levels into the staging area
             // (which aliases the ring: all targets of the levels p >= 1 belong to the last pass, whose ring is idle now)
-            static_for<0, NC>([&](auto iw) {
-                constexpr int w = decltype(iw)::value;
-                static_assert(T0 + w < NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
-                if (warp == w) target_drop<LX, LA, LB, T0 + w>(acc, TC, ZB, lane);
-            });
+            static_assert(T0 + NC <= NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
+            if (warp < NC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
             __syncthreads();
         });
-        chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, warp, lane, batch, map, aux, prim, out, swapped, df);
+        chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
     }
 }
 

@@ -189,29 +189,57 @@ __host__ __device__ constexpr int target_index(int LX, int p, int g) {
     return o + g - off(LX - 2 * p);
 }
 
-// Drop the contracted target TI of this lane's set: level 0 goes straight to its Cartesian slot of TC, higher levels to
-// the staging area UB[(ti − NXC)][i][lane]; both scaled back by a! (lx_chain.cuh header).
-template <int LX, int LA, int LB, int TI>
-__device__ __forceinline__ void target_drop(const double *__restrict__ acc, double *__restrict__ TC, double *__restrict__ UB, int lane) {
+// Partner table of the gather step, built once per block in shared memory by compile-time unrolled stores:
+// for every Cartesian c the targets (level p >= 1, t = c − 2n) that contribute, with their integer weights β(c,n).
+constexpr int CHAIN_MAXPART = 8;
+struct PartnerTab {
+    int cnt[nc(LX_MAX_L_AUX)];
+    int ti[nc(LX_MAX_L_AUX)][CHAIN_MAXPART];
+    int beta[nc(LX_MAX_L_AUX)][CHAIN_MAXPART];
+};
+template <int LX>
+__device__ __forceinline__ void partner_tab_build(PartnerTab *pt) {
+    static_for<0, nc(LX)>([&](auto ic) {
+        constexpr int c = decltype(ic)::value, gc = off(LX) + c;
+        constexpr int cx = cart_pow(gc, 0), cy = cart_pow(gc, 1), cz = cart_pow(gc, 2);
+        int k = 0;
+        static_for<0, cx / 2 + 1>([&](auto inx) {
+            static_for<0, cy / 2 + 1>([&](auto iny) {
+                static_for<0, cz / 2 + 1>([&](auto inz) {
+                    constexpr int nx = decltype(inx)::value, ny = decltype(iny)::value, nz = decltype(inz)::value;
+                    if constexpr (nx + ny + nz > 0) {
+                        pt->ti[c][k] = target_index(LX, nx + ny + nz, cart_index(cx - 2 * nx, cy - 2 * ny, cz - 2 * nz));
+                        pt->beta[c][k] = beta1(cx, nx) * beta1(cy, ny) * beta1(cz, nz);
+                        ++k;
+                    }
+                });
+            });
+        });
+        pt->cnt[c] = k;
+    });
+}
+
+// Drop the contracted target ti (run-time, warp-uniform) of this lane's set: level 0 goes straight to its Cartesian slot
+// of TC, higher levels to the staging area UB[(ti − NXC)][i][lane]; both scaled back by a! (lx_chain.cuh header).
+// One copy of this code serves every target: code that runs once per batch must stay small (instruction cache).
+template <int LX, int LA, int LB>
+__device__ __forceinline__ void target_drop(int ti, const double *__restrict__ acc, double *__restrict__ TC,
+                                            double *__restrict__ UB, int lane) {
     using CC = ChainCls<LX, LA, LB>;
     constexpr int NACC = CC::NACC, NXC = CC::NXC;
-    if constexpr (TI < NXC) {
-        static_for<0, NACC>([&](auto ii) {
-            constexpr int i = decltype(ii)::value;
-            TC[(size_t)lane * CC::SLOTN + TI * CC::NAB + i] = acc[i] * (double)cart_fact(off(LA) + i);
-        });
-    } else {
-        static_for<0, NACC>([&](auto ii) {
-            constexpr int i = decltype(ii)::value;
-            UB[((size_t)(TI - NXC) * NACC + i) * 32 + lane] = acc[i] * (double)cart_fact(off(LA) + i);
-        });
-    }
+    double *dst = ti < NXC ? TC + (size_t)lane * CC::SLOTN + ti * CC::NAB : UB + (size_t)(ti - NXC) * NACC * 32 + lane;
+    const int stride = ti < NXC ? 1 : 32;
+    static_for<0, NACC>([&](auto ii) {
+        constexpr int i = decltype(ii)::value;
+        dst[i * stride] = acc[i] * (double)cart_fact(off(LA) + i);
+    });
 }
 
 // After the targets of a batch were dropped (and a block barrier): gather (e0|c) = U_{0,c} + Σ_{n>0} β(c,n) U_{|n|,c−2n},
 // HRR in registers per (set = lane, c) in place in TC, then one warp per set stores / digests the finished shell-set.
 template <int LX, int LA, int LB, int MODE, int NW>
-__device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const double *__restrict__ UB, int warp, int lane,
+__device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const double *__restrict__ UB,
+                                               const PartnerTab *__restrict__ pt, int warp, int lane,
                                                long long batch, const SetMap &map, const DevShells &aux,
                                                const DevShells &prim, double *__restrict__ out, int swapped, const DfArgs &df) {
     using CC = ChainCls<LX, LA, LB>;
@@ -223,29 +251,23 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
         double AB[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) AB[d] = prim.center[3 * sid.a + d] - prim.center[3 * sid.b + d];
-        static_for<0, NXC>([&](auto ic) {
-            constexpr int c = decltype(ic)::value, gc = off(LX) + c;
-            if (warp == c % NW) {
+        for (int c = warp; c < NXC; c += NW) {               // run-time c: one copy of the code
+            {
                 double *reg = TC + (size_t)lane * SLOTN + c * NAB;
                 double H0[NACC];
                 static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = reg[decltype(ii)::value]; });
-                constexpr int cx = cart_pow(gc, 0), cy = cart_pow(gc, 1), cz = cart_pow(gc, 2);
-                static_for<0, cx / 2 + 1>([&](auto inx) {
-                    static_for<0, cy / 2 + 1>([&](auto iny) {
-                        static_for<0, cz / 2 + 1>([&](auto inz) {
-                            constexpr int nx = decltype(inx)::value, ny = decltype(iny)::value, nz = decltype(inz)::value;
-                            constexpr int p = nx + ny + nz;
-                            if constexpr (p > 0) {
-                                constexpr int ti = target_index(LX, p, cart_index(cx - 2 * nx, cy - 2 * ny, cz - 2 * nz));
-                                constexpr double beta = (double)(beta1(cx, nx) * beta1(cy, ny) * beta1(cz, nz));
-                                static_for<0, NACC>([&](auto ii) {
-                                    constexpr int i = decltype(ii)::value;
-                                    H0[i] = fma(beta, UB[((size_t)(ti - NXC) * NACC + i) * 32 + lane], H0[i]);
-                                });
-                            }
+                if constexpr (LX >= 2) {
+                    const int np_ = pt->cnt[c];
+#pragma unroll 1
+                    for (int k = 0; k < np_; ++k) {
+                        const double beta = (double)pt->beta[c][k];
+                        const double *ub = UB + (size_t)(pt->ti[c][k] - NXC) * NACC * 32 + lane;
+                        static_for<0, NACC>([&](auto ii) {
+                            constexpr int i = decltype(ii)::value;
+                            H0[i] = fma(beta, ub[i * 32], H0[i]);
                         });
-                    });
-                });
+                    }
+                }
                 if constexpr (LB == 0) {
                     static_for<0, NACC>([&](auto ii) { reg[decltype(ii)::value] = H0[decltype(ii)::value]; });
                 } else {
@@ -274,10 +296,38 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
                     }
                 }
             }
-        });
+        }
         __syncthreads();
     }
-    for (int s = warp; s < 32; s += NW) {
+    if constexpr (MODE == 0) {
+        // a8: the batch is one contiguous run of out[]; all warps copy it, four independent elements in flight per lane
+        const long long nlive = min((long long)32, map.nsets - batch * 32);
+        const int total = (int)nlive * NINT;
+        double *o = out + batch * 32 * NINT;
+        const int tid = warp * 32 + lane;
+        for (int it0 = tid; it0 < total; it0 += NW * 32 * 4) {
+            double v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int it = it0 + u * NW * 32;
+                if (it < total) {
+                    const int sset = it / NINT, r = it - sset * NINT;
+                    int src = r;
+                    if (swapped && LB > 0) {                  // caller's order is [c][b][a]
+                        const int ia = r % NA, t = r / NA, ib = t % NB, c = t / NB;
+                        src = (c * NA + ia) * NB + ib;
+                    }
+                    v[u] = TC[(size_t)sset * SLOTN + src];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int it = it0 + u * NW * 32;
+                if (it < total) o[it] = v[u];
+            }
+        }
+    }
+    for (int s = warp; MODE != 0 && s < 32; s += NW) {
         const long long sid_s = batch * 32 + s;
         if (sid_s >= map.nsets) break;                    // warp-uniform
         const double *FIN = TC + (size_t)s * SLOTN;       // finished shell-set, layout [c][a][b]
@@ -330,7 +380,7 @@ struct TeamCls {
     using CC = ChainCls<LX, LA, LB>;
     static constexpr int NT = CC::T.n, NTW = (NT + W - 1) / W;
     static constexpr int NUB = (NT - CC::NXC) * CC::NACC * 32;            // staging of the levels p >= 1
-    static constexpr size_t smem = ((size_t)32 * CC::SLOTN + NUB + 4) * 8;
+    static constexpr size_t smem = ((size_t)32 * CC::SLOTN + NUB + 4) * 8 + sizeof(PartnerTab);
     static constexpr int acc_doubles = NTW * CC::NACC;                   // accumulators a lane keeps
 };
 // smallest team whose lanes keep at most `budget` accumulator doubles (0 = none fits in 8 warps)
@@ -355,6 +405,9 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]
     double *UB = TC + (size_t)32 * CC::SLOTN;                // [(ti − NXC)][i][set]
+    PartnerTab *pt = reinterpret_cast<PartnerTab *>(UB + TM::NUB + 4);
+    if (threadIdx.x == 0) partner_tab_build<LX>(pt);
+    __syncthreads();
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long nbatch = (map.nsets + 31) / 32;
@@ -419,13 +472,13 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                     }
                     static_for<T0, T1>([&](auto it) {
                         constexpr int ti = decltype(it)::value;
-                        target_drop<LX, LA, LB, ti>(acc + (ti - T0) * NACC, TC, UB, lane);
+                        target_drop<LX, LA, LB>(ti, acc + (ti - T0) * NACC, TC, UB, lane);
                     });
                 }
             }
         });
         __syncthreads();
-        chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, warp, lane, batch, map, aux, prim, out, swapped, df);
+        chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
     }
 }
 
