@@ -13,6 +13,10 @@ LIB = os.path.join(HERE, "liblx.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
+# tuning aid: extra nvcc flags (e.g. "-DLX_TEAM_BUDGET=40") from the environment; they force a rebuild
+EXTRA = os.environ.get("LX_EXTRA_NVCC", "").split()
+NVCC_FLAGS += EXTRA
+
 LX_RANGE = range(7)      # aux angular momentum 0..LX_MAX_L_AUX
 MODES = range(3)         # 0 store, 1 gamma, 2 J
 
@@ -50,7 +54,7 @@ def build(verbose=False, force=False, jobs=None):
         o = os.path.join(OBJ, obj)
         s = os.path.join(CSRC, src)
         objs.append(o)
-        if force or _stale(o, [s] + hdrs):
+        if force or EXTRA or _stale(o, [s] + hdrs):
             todo.append(["nvcc"] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
 
     def run(cmd):

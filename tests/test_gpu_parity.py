@@ -201,3 +201,30 @@ def test_df_no_screening_and_subset_pairs(lx, oracle):
     J = lx.lx_df_J(sched, da, dp, torch.from_numpy(d).cuda()).cpu().numpy()
     assert np.linalg.norm(gamma - g_ref) <= 1e-11 * np.linalg.norm(g_ref)
     assert np.linalg.norm(J - J_ref) <= 1e-11 * np.linalg.norm(J_ref)
+
+
+@pytest.mark.parametrize("cls", [(4, 2, 2), (4, 1, 2), (3, 2, 1), (2, 1, 1), (3, 2, 0), (0, 0, 0), (4, 0, 0), (1, 2, 2)])
+def test_config2_full_size_sampled(lx, oracle, cls):
+    """BASELINE.json configs[1] at full size (1024 pairs x 256 aux shells, the launch configuration bench.py times):
+    the whole batch runs on the GPU; seeded samples of (pair, aux) blocks are checked element by element against the
+    oracle, which evaluates exactly those shell-sets.  Covers the team, chain and mirrored (la < lb) paths."""
+    lxa, la, lb = cls
+    cfg = gen.config2(lxa, la, lb)
+    got = _run(lx, cfg)
+    assert got.shape[:2] == (1024, 256)
+    assert np.isfinite(got).all()
+    rng = np.random.default_rng(7)
+    ps = np.sort(rng.choice(1024, size=12, replace=False))
+    xs = np.sort(rng.choice(256, size=24, replace=False))
+    ps[0], ps[-1], xs[0], xs[-1] = 0, 1023, 0, 255                       # first and last block of the batch
+    ref = oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"][xs], cfg["pair_idx"][ps])
+    sub = got[np.ix_(ps, xs)]
+    scale = np.max(np.abs(got))
+    assert np.max(np.abs(sub - ref)) <= TOL * scale
+
+
+def test_kernel_families_cover_config2(lx):
+    """Every class of the class sweep runs on one of the register-resident families (no silent fallback)."""
+    fams = {c: lx.lx_kernel_family(*c) for c in gen.CONFIG2_CLASSES}
+    assert set(fams.values()) <= {"team", "chain"}, fams
+    assert fams[(4, 2, 2)] == "chain" and fams[(2, 1, 1)] == "team"
