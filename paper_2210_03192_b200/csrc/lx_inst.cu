@@ -16,8 +16,11 @@ namespace lx {
 // kernel family per class: team kernel where the chain targets of a warp fit its registers,
 // warp-specialised chain kernel for the other classes with La+Lb <= 4 and Lx <= 4, lane / group kernels beyond.
 // LX_FAMILY=team|chain|lane in the environment overrides the choice where the named family exists (tuning aid).
+#ifndef LX_TEAM_WMAX
+#define LX_TEAM_WMAX 2
+#endif
 #ifndef LX_TEAM_BUDGET
-#define LX_TEAM_BUDGET 56
+#define LX_TEAM_BUDGET 72
 #endif
 static int family_override() {
     static int v = -1;
@@ -35,7 +38,7 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
     constexpr bool small = LA + LB <= 4 && LX <= 4;
     constexpr int TW = small ? team_size(LX, LA, LB, LX_TEAM_BUDGET) : 0;
     // measured (config 2, B200): the team kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets
-    constexpr bool has_team = TW > 0 && (LA + LB <= 2 || TW <= 2), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
+    constexpr bool has_team = TW > 0 && (LA + LB <= 2 || TW <= LX_TEAM_WMAX), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
     const int ov = family_override();
     if constexpr (has_team) {
         if (ov == 0 || ov == 1 || (ov == 2 && !has_chain) || (ov == 3 && !has_lane))
