@@ -30,6 +30,8 @@ METRIC = "3-center integrals/sec (class sweep, config 2)"
 UNIT = "integrals/s"
 WORKLOAD = "configs[1]: 45 classes (Lx 0..4 | La,Lb 0..2), K_total=9, 1024 pairs x 256 aux per class"
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk/SM x 2 x sm_max_mhz
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures under profiles/ (class -> bytes)
+NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): 1.083989e9 + 0.964e6}   # profiles/r01_ncu_chain_4_2_2.md
 # SURVEY.md §8(d) table, flops per shell-set at K = 9 for the classes it lists
 SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
                         (4, 1, 1): 29322, (4, 2, 2): 111054}
@@ -255,15 +257,15 @@ def main():
         c_top = classes[i_top]
         canon = (c_top[0], max(c_top[1:]), min(c_top[1:]))
         # algorithmic flops per shell-set: the component-level DAG count of costmodel.py; SURVEY.md
-        # §8(d) quotes a larger figure for some classes (it over-counts: ncu's executed DFMA/DMUL/DADD count matches
-        # the cost model, profiles/r01_ncu_lane_4_2_2.md) and is reported next to it
+        # §8(d) quotes a larger figure for some classes (it over-counts: ncu's executed DFMA/DMUL/DADD count of the
+        # full-OS lane kernel matches the cost model, profiles/r01_ncu_lane_4_2_2.md) and is reported next to it
         fl_set = costmodel.flops_per_set(*c_top, 9)
         fl_survey = SURVEY_FLOPS_PER_SET.get(canon)
         t_top = class_ms[i_top] * 1e-3
         achieved = fl_set * nsets / t_top / 1e12
         roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family(*canon)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
                     "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
-                    "traffic": None, "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(canon), "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
                     "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
                     "flops_per_set_survey": fl_survey,
                     "frac_with_survey_flops": (fl_survey * nsets / t_top / 1e12 / FP64_NOMINAL_TFLOPS) if fl_survey else None,
