@@ -81,7 +81,8 @@ struct ChainPlan {
     int plo[CHAIN_MAXPASS], phi[CHAIN_MAXPASS];     // levels the pass needs
     int nprod[CHAIN_MAXPASS];                       // producer warps of the pass
     int nw;                                         // warps per block
-    int ring;                                       // doubles of the largest ring (producers + 1 buffers)
+    int ring;                                       // doubles of the ring (npx + 1 buffers of zrec doubles)
+    int ncx, npx, zrec;                             // consumer / producer warps of the block, doubles per ring buffer
     bool ok;                                        // every target of a level p >= 1 sits in the last pass
 };
 // doubles of one ring buffer of a pass over nlev levels: start vectors [level][g][32], r[3][32], ck[level][32]
@@ -96,7 +97,8 @@ constexpr ChainPlan chain_plan(int LX, int LA, int LB) {
     ChainPlan P{};
     P.npass = (T.n + cap - 1) / cap;
     const int ncw = (T.n + P.npass - 1) / P.npass;
-    P.nw = 0; P.ring = 0; P.ok = true;
+    P.nw = 0; P.ring = 0; P.ok = true; P.ncx = 0; P.npx = 0;
+    int nlevx = 0;
     for (int i = 0; i < P.npass; ++i) {
         // even split, except that the targets of the levels p >= 1 (index >= nc(LX)) all go to the last pass
         P.t0[i] = i == 0 ? 0 : P.t1[i - 1];
@@ -111,13 +113,18 @@ constexpr ChainPlan chain_plan(int LX, int LA, int LB) {
         const int prod = nlev * (4 * chain_nv1(E) + 2 * NG + 60) + 130;
         int np = (prod + cons - 1) / cons;
         np = cmax(1, cmin(np, cmin(6, nwmax - (P.t1[i] - P.t0[i]))));
-        // the ring shares 227 KB with the (e0|c) region of the 32 sets and the header
-        const int room = (227 * 1024) / 8 - 32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) - 520 - 256;
-        while (np > 1 && (np + 1) * chain_zrec(nlev, NG) > room) --np;
         P.nprod[i] = np;
-        P.nw = cmax(P.nw, P.t1[i] - P.t0[i] + np);
-        P.ring = cmax(P.ring, (np + 1) * chain_zrec(nlev, NG));
+        P.ncx = cmax(P.ncx, P.t1[i] - P.t0[i]);
+        P.npx = cmax(P.npx, np);
+        nlevx = cmax(nlevx, nlev);
     }
+    // one ring for all passes; it shares 227 KB with the (e0|c) region of the 32 sets, the header and two small tables
+    P.npx = cmin(P.npx, nwmax - P.ncx);
+    P.zrec = chain_zrec(nlevx, NG);
+    const int room = (227 * 1024) / 8 - 32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) - 520 - 256;
+    while (P.npx > 1 && (P.npx + 1) * P.zrec > room) --P.npx;
+    P.nw = P.ncx + P.npx;
+    P.ring = (P.npx + 1) * P.zrec;
     return P;
 }
 

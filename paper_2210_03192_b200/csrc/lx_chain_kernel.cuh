@@ -73,26 +73,30 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         __syncthreads();
         const int kmax = *s_kmax;
 
-        // ---- passes over the primitive loop --------------------------------------------------------------------------------
-        static_for<0, P.npass>([&](auto ipass) {
-            constexpr int ip = decltype(ipass)::value;
-            constexpr int T0 = P.t0[ip], NC = P.t1[ip] - P.t0[ip], PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
-            constexpr int NPROD = P.nprod[ip], NBUF = NPROD + 1, ZREC = chain_zrec(NLV, NG);
-            constexpr int BCOUNT = (NC + 1) * 32;            // threads on a full[] / empty[] barrier
-            double acc[NACC];
-#pragma unroll
-            for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
-
-            if (warp >= NC && warp < NC + NPROD) {
-                // ================= producer: primitives q = j, j + NPROD, ... =================================================
-                const int j = warp - NC;
-                const double Ax = hd[0 * 32 + lane], Ay = hd[1 * 32 + lane], Az = hd[2 * 32 + lane];
-                const double Cx = hd[3 * 32 + lane], Cy = hd[4 * 32 + lane], Cz = hd[5 * 32 + lane];
-                const long long po = hpo[lane];
-                const int xo0 = hi[0 * 32 + lane], Kab = hi[1 * 32 + lane], K = hi[2 * 32 + lane];
-                for (int q = j; q < kmax; q += NPROD) {
-                    const int bsel = q % NBUF;
-                    if (q >= NBUF) named_sync(1 + NBUF + bsel, BCOUNT);      // consumers are done with this buffer
+        // ---- passes over the primitive loop: ONE ring runs through all passes (slot g = pass * kmax + q), so the producers
+        // of pass i+1 fill it while the consumers of pass i finish; roles are fixed for the batch: warps [0, NCX) consume
+        // (warp w holds target T0 + w of the current pass, or idles through the barriers), warps [NCX, NCX + NPX) produce.
+        constexpr int NCX = P.ncx, NPX = P.npx, NBUF = NPX + 1, ZREC = P.zrec;
+        constexpr int BCOUNT = (NCX + 1) * 32;               // threads on a full[] / empty[] barrier
+        // measured: with three or more passes the producers running ahead into the code of the next pass cost more
+        // (instruction cache) than the pipeline refill they save, so those classes re-align at every pass boundary
+        constexpr bool CONT = P.npass <= 2;
+        const int gtot = P.npass * kmax;                     // ring slots of the batch
+        double acc[NACC];
+        if (warp >= NCX) {
+            // ================= producers: ring slots g = j, j + NPX, ... ======================================================
+            const int j = warp - NCX;
+            const double Ax = hd[0 * 32 + lane], Ay = hd[1 * 32 + lane], Az = hd[2 * 32 + lane];
+            const double Cx = hd[3 * 32 + lane], Cy = hd[4 * 32 + lane], Cz = hd[5 * 32 + lane];
+            const long long po = hpo[lane];
+            const int xo0 = hi[0 * 32 + lane], Kab = hi[1 * 32 + lane], K = hi[2 * 32 + lane];
+            static_for<0, P.npass>([&](auto ipass) {
+                constexpr int ip = decltype(ipass)::value;
+                constexpr int PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
+                const int g0 = ip * kmax;
+                for (int q = ((j - g0) % NPX + NPX) % NPX; q < kmax; q += NPX) {
+                    const int g = g0 + q, bsel = g % NBUF;
+                    if (g >= NBUF) named_sync(1 + NBUF + bsel, BCOUNT);      // consumers are done with this buffer
                     double *zb = ZB + (size_t)bsel * ZREC;
                     const bool on = q < K;
                     const int qq = on ? q : 0;
@@ -187,10 +191,19 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                     __threadfence_block();
                     named_arrive(1 + bsel, BCOUNT);           // full[bsel]
                 }
-            } else if (warp < NC) {
-                // ================= consumer: target T0 + warp ====================================================================
+                if constexpr (!CONT && ip + 1 < P.npass) named_sync(15, NW * 32);
+            });
+        } else {
+            // ================= consumers ===========================================================================================
+            static_for<0, P.npass>([&](auto ipass) {
+                constexpr int ip = decltype(ipass)::value;
+                constexpr int T0 = P.t0[ip], NC = P.t1[ip] - P.t0[ip], PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
+                static_assert(T0 + NC <= NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+                const int g0 = ip * kmax;
                 for (int q = 0; q < kmax; ++q) {
-                    const int bsel = q % NBUF;
+                    const int g = g0 + q, bsel = g % NBUF;
                     named_sync(1 + bsel, BCOUNT);             // full[bsel]
                     const double *zb = ZB + (size_t)bsel * ZREC;
                     const double *rec = zb + (size_t)NLV * NG * 32;
@@ -202,16 +215,20 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                             chain_apply<LA, E, cart_pow(tg, 0), cart_pow(tg, 1), cart_pow(tg, 2)>(zb + (size_t)lv * NG * 32, lane, rx, ry, rz, ck, acc);
                         }
                     });
-                    if (q + NBUF < kmax) named_arrive(1 + NBUF + bsel, BCOUNT);   // empty[bsel]
+                    if (g + NBUF < gtot) named_arrive(1 + NBUF + bsel, BCOUNT);   // empty[bsel]
                 }
-            }
-            __syncthreads();
-            // ---- drop the contracted targets: level 0 into its Cartesian slot of TC, higher levels into the staging area
-            // (which aliases the ring: all targets of the levels p >= 1 belong to the last pass, whose ring is idle now)
-            static_assert(T0 + NC <= NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
-            if (warp < NC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
-            __syncthreads();
-        });
+                // level-0 targets go straight to their private Cartesian slot of TC
+                if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
+                if constexpr (!CONT && ip + 1 < P.npass) named_sync(15, NW * 32);
+            });
+        }
+        __syncthreads();
+        // the targets of the levels p >= 1 (all in the last pass) go to the staging area, which aliases the now idle ring
+        if constexpr (CC::T.n > NXC) {
+            constexpr int T0L = P.t0[P.npass - 1], NCL = P.t1[P.npass - 1] - T0L;
+            if (warp < NCL && T0L + warp >= NXC) target_drop<LX, LA, LB>(T0L + warp, acc, TC, ZB, lane);
+        }
+        __syncthreads();
         chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
     }
 }
