@@ -143,6 +143,7 @@ def main():
     ap.add_argument("--classes", default="", help="profiling aid: restrict the sweep to e.g. '4,2,1;4,0,0' (default: all 45)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-df", action="store_true", help="skip the DF-J (config 4) side measurement")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -280,6 +281,33 @@ def main():
             n, t, cores = oracle_sample(classes, npair_s, nx_s, seed=2)
             cpu = {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
                    "sample": f"first {npair_s} pairs x {nx_s} aux shells of each of the 45 classes ({n} integrals, {t:.1f} s)"}
+        # ---- side measurement (BASELINE.json metric "DF-J time"): integral-direct gamma and J on configs[3] (64 atoms,
+        # 960 AO x 6 784 Cartesian DFAO) through lx_df_gamma / lx_df_J, all shell-sets (Schwarz factors are oracle data:
+        # the screened path is covered by the parity tests, not timed here); not part of `value`
+        df = None
+        if world == 1 and not args.no_df and not args.classes:
+            c4 = gen.config4()
+            h4a, h4p = lx.HostShells(c4["aux"]), lx.HostShells(c4["prim"])
+            sched = lx.Schedule(h4a, h4p, None, None, c4["pair_idx"], 0.0)
+            d4a, d4p = lx.DeviceShells(h4a, dev), lx.DeviceShells(h4p, dev)
+            D4, v4 = torch.from_numpy(c4["D"]).to(dev), torch.from_numpy(c4["d"]).to(dev)
+            ms = {}
+            for name, fn, arg in (("gamma", lx.lx_df_gamma, D4), ("J", lx.lx_df_J, v4)):
+                fn(sched, d4a, d4p, arg)
+                torch.cuda.synchronize()
+                best = 1e30
+                for _ in range(3):
+                    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a0.record()
+                    fn(sched, d4a, d4p, arg)
+                    a1.record()
+                    torch.cuda.synchronize()
+                    best = min(best, a0.elapsed_time(a1))
+                ms[name] = best
+            df = {"workload": "configs[3]: 64-atom cluster, nbf 960, naux 6784 (Cartesian), 73920 unique shell pairs x 1344 aux shells",
+                  "screening": "none (all shell-sets computed)", "shell_sets": sched.num_sets, "integrals": sched.num_integrals,
+                  "gamma_ms": ms["gamma"], "J_ms": ms["J"], "df_j_ms": ms["gamma"] + ms["J"],
+                  "integrals_per_s": 2 * sched.num_integrals / ((ms["gamma"] + ms["J"]) * 1e-3)}
         per_class = {f"({c[0]}|{c[1]}{c[2]})": round(float(nint_set(c) * nsets / (m * 1e-3)), 1) for c, m in zip(classes, class_ms)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -290,7 +318,7 @@ def main():
                                  f"{ints_per_step * 8 / 1e9:.1f} GB of output",
                            "parallelism": f"{world} x independent batch (no collective)"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-                "shell_sets_per_s": value / ints_per_step * nsets * len(classes),
+                "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df,
                 "integrals_per_s_per_class": per_class}
         print(json.dumps(line))
     if world > 1:
