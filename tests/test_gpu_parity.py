@@ -228,3 +228,14 @@ def test_kernel_families_cover_config2(lx):
     fams = {c: lx.lx_kernel_family(*c) for c in gen.CONFIG2_CLASSES}
     assert set(fams.values()) <= {"team", "chain"}, fams
     assert fams[(4, 2, 2)] == "chain" and fams[(2, 1, 1)] == "team"
+
+
+@pytest.mark.parametrize("cls", [(4, 2, 2), (3, 2, 0)])
+def test_store_mode_is_deterministic(lx, cls):
+    """MODE 0 has no atomics: two runs of the same batch must agree bit for bit (compute-sanitizer is closed on this
+    pool, so this and the element-wise parity are the race checks for the named-barrier ring of the chain kernel and
+    the shared-memory epilogue)."""
+    cfg = gen.config2(*cls, npair=64, nx=96)
+    a = _run(lx, cfg)
+    for _ in range(3):
+        assert np.array_equal(a, _run(lx, cfg))
