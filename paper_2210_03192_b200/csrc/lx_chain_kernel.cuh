@@ -80,7 +80,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         constexpr int BCOUNT = (NCX + 1) * 32;               // threads on a full[] / empty[] barrier
         // measured: with three or more passes the producers running ahead into the code of the next pass cost more
         // (instruction cache) than the pipeline refill they save, so those classes re-align at every pass boundary
-        constexpr bool CONT = P.npass <= 2;
+        // (CONT = npass <= 2)
         const int gtot = P.npass * kmax;                     // ring slots of the batch
         double acc[NACC];
         if (warp >= NCX) {
@@ -191,7 +191,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                     __threadfence_block();
                     named_arrive(1 + bsel, BCOUNT);           // full[bsel]
                 }
-                if constexpr (!CONT && ip + 1 < P.npass) named_sync(15, NW * 32);
+                if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
             });
         } else {
             // ================= consumers ===========================================================================================
@@ -219,7 +219,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 }
                 // level-0 targets go straight to their private Cartesian slot of TC
                 if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
-                if constexpr (!CONT && ip + 1 < P.npass) named_sync(15, NW * 32);
+                if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
             });
         }
         __syncthreads();
