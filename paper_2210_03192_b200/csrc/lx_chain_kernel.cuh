@@ -82,7 +82,6 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         // (instruction cache) than the pipeline refill they save, so those classes re-align at every pass boundary
         // (CONT = npass <= 2)
         const int gtot = P.npass * kmax;                     // ring slots of the batch
-        double acc[NACC];
         if (warp >= NCX) {
             // ================= producers: ring slots g = j, j + NPX, ... ======================================================
             const int j = warp - NCX;
@@ -193,8 +192,10 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 }
                 if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
             });
+            named_sync(15, NW * 32);                         // all ring traffic of the batch is done
         } else {
             // ================= consumers ===========================================================================================
+            double acc[NACC];                                // lives in the consumer branch only: producers keep their registers
             static_for<0, P.npass>([&](auto ipass) {
                 constexpr int ip = decltype(ipass)::value;
                 constexpr int T0 = P.t0[ip], NC = P.t1[ip] - P.t0[ip], PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
@@ -221,12 +222,12 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
                 if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
             });
-        }
-        __syncthreads();
-        // the targets of the levels p >= 1 (all in the last pass) go to the staging area, which aliases the now idle ring
-        if constexpr (CC::T.n > NXC) {
-            constexpr int T0L = P.t0[P.npass - 1], NCL = P.t1[P.npass - 1] - T0L;
-            if (warp < NCL && T0L + warp >= NXC) target_drop<LX, LA, LB>(T0L + warp, acc, TC, ZB, lane);
+            named_sync(15, NW * 32);                         // all ring traffic of the batch is done
+            // the targets of the levels p >= 1 (all in the last pass) go to the staging area, which aliases the idle ring
+            if constexpr (CC::T.n > NXC) {
+                constexpr int T0L = P.t0[P.npass - 1], NCL = P.t1[P.npass - 1] - T0L;
+                if (warp < NCL && T0L + warp >= NXC) target_drop<LX, LA, LB>(T0L + warp, acc, TC, ZB, lane);
+            }
         }
         __syncthreads();
         chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
