@@ -3,6 +3,10 @@
 #pragma once
 #include "lx_team.cuh"
 
+#ifndef LX_CHAIN_REALIGN
+#define LX_CHAIN_REALIGN 1
+#endif
+
 namespace lx {
 
 template <int LX, int LA, int LB, int MODE, int NW, int MINB>
@@ -190,7 +194,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                     __threadfence_block();
                     named_arrive(1 + bsel, BCOUNT);           // full[bsel]
                 }
-                if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
+                if constexpr (LX_CHAIN_REALIGN && CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);
             });
             named_sync(15, NW * 32);                         // all ring traffic of the batch is done
         } else {
@@ -220,7 +224,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                 }
                 // level-0 targets go straight to their private Cartesian slot of TC
                 if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
-                if constexpr (CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);   // !CONT
+                if constexpr (LX_CHAIN_REALIGN && CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);
             });
             named_sync(15, NW * 32);                         // all ring traffic of the batch is done
             // the targets of the levels p >= 1 (all in the last pass) go to the staging area, which aliases the idle ring
