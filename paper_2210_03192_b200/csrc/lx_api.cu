@@ -166,8 +166,9 @@ const char *lx_kernel_family(int lx_, int la, int lb) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
     {
         const int ca = std::max(la, lb), cb = std::min(la, lb);
-        const int tw = (ca + cb <= 4) ? team_size(lx_, ca, cb, 72) : 0;
-        if (tw > 0 && (lx_ <= 4 ? (ca + cb <= 2 || tw <= 2) : (ca + cb >= 1 && tw <= 3))) return "team";
+        const bool wide = lx_ == 3 && ca == 2 && cb == 1;
+        const int tw = (ca + cb <= 4) ? team_size(lx_, ca, cb, wide ? 80 : 72) : 0;
+        if (tw > 0 && (lx_ <= 4 ? (ca + cb <= 2 || tw <= (wide ? 3 : 2)) : (ca + cb >= 1 && tw <= 3))) return "team";
         if (chain_fits(lx_, ca, cb)) return "chain";
     }
     return lane_fits(std::max(la, lb), std::min(la, lb)) ? "lane" : "group";

@@ -36,10 +36,12 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
                                 const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                                 cudaStream_t stream) {
     constexpr bool small = LA + LB <= 4 && LX <= LX_MAX_L_AUX;   // team: any Lx; the chain kernel has its own bound (Lx <= 4)
-    constexpr int TW = small ? team_size(LX, LA, LB, LX_TEAM_BUDGET) : 0;
+    // (3|21) keeps all 13 targets in three warps with 80 accumulator doubles per lane: measured faster than the chain kernel
+    constexpr bool wide = LX == 3 && LA == 2 && LB == 1;
+    constexpr int TW = small ? team_size(LX, LA, LB, wide ? 80 : LX_TEAM_BUDGET) : 0;
     // measured (B200): for Lx <= 4 the team kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets;
     // for Lx = 5, 6 it beats the lane kernel while at most three warps hold the targets
-    constexpr bool has_team = TW > 0 && (LX <= 4 ? (LA + LB <= 2 || TW <= LX_TEAM_WMAX) : (LA + LB >= 1 && TW <= 3)), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
+    constexpr bool has_team = TW > 0 && (LX <= 4 ? (LA + LB <= 2 || TW <= (wide ? 3 : LX_TEAM_WMAX)) : (LA + LB >= 1 && TW <= 3)), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
     const int ov = family_override();
     if constexpr (has_team) {
         if (ov == 0 || ov == 1 || (ov == 2 && !has_chain) || (ov == 3 && !has_lane))

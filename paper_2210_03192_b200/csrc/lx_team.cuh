@@ -247,6 +247,8 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
     constexpr int NINT = CC::NINT, SLOTN = CC::SLOTN;
     constexpr unsigned FULL = 0xffffffffu;
     const SetId sid = decode_set(map, batch * 32 + lane, swapped);
+    // a mirrored class (caller's order [c][b][a]) gets its shell-sets transposed by the HRR stores, not by the copy-out
+    const bool tr = MODE == 0 && swapped != 0;
     if constexpr (LB > 0 || LX >= 2) {
         double AB[3];
 #pragma unroll
@@ -281,7 +283,10 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
                         });
                     });
                     if constexpr (LB == 1) {
-                        static_for<0, NA * 3>([&](auto ii) { reg[decltype(ii)::value] = H1[decltype(ii)::value]; });
+                        static_for<0, NA * 3>([&](auto ii) {
+                            constexpr int i = decltype(ii)::value;
+                            reg[tr ? (i % 3) * NA + i / 3 : i] = H1[i];
+                        });
                     } else {
                         static_assert(LB <= 2, "chain epilogue: HRR written for Lb <= 2");
                         static_for<0, NA>([&](auto ial) {
@@ -290,7 +295,7 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
                                 constexpr int bj = decltype(ib)::value, gb = off(2) + bj;
                                 constexpr int d = (int)(cart_entry(gb) >> 24);
                                 constexpr int b1 = cart_dn(gb, d) - off(1);
-                                reg[al * 6 + bj] = fma(AB[d], H1[al * 3 + b1], H1[(cart_up(g, d) - off(LA)) * 3 + b1]);
+                                reg[tr ? bj * NA + al : al * 6 + bj] = fma(AB[d], H1[al * 3 + b1], H1[(cart_up(g, d) - off(LA)) * 3 + b1]);
                             });
                         });
                     }
@@ -312,12 +317,7 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
                 const int it = it0 + u * NW * 32;
                 if (it < total) {
                     const int sset = it / NINT, r = it - sset * NINT;
-                    int src = r;
-                    if (swapped && LB > 0) {                  // caller's order is [c][b][a]
-                        const int ia = r % NA, t = r / NA, ib = t % NB, c = t / NB;
-                        src = (c * NA + ia) * NB + ib;
-                    }
-                    v[u] = TC[(size_t)sset * SLOTN + src];
+                    v[u] = TC[(size_t)sset * SLOTN + r];
                 }
             }
 #pragma unroll
@@ -331,17 +331,7 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
         const long long sid_s = batch * 32 + s;
         if (sid_s >= map.nsets) break;                    // warp-uniform
         const double *FIN = TC + (size_t)s * SLOTN;       // finished shell-set, layout [c][a][b]
-        if constexpr (MODE == 0) {
-            double *o = out + sid_s * NINT;
-            if (!swapped || LB == 0) {
-                for (int r = lane; r < NINT; r += 32) o[r] = FIN[r];
-            } else {                                      // caller's order is [c][b][a]
-                for (int r = lane; r < NINT; r += 32) {
-                    const int ia = r % NA, t = r / NA, ib = t % NB, c = t / NB;
-                    o[r] = FIN[(c * NA + ia) * NB + ib];
-                }
-            }
-        } else {
+        {
             const int as = __shfl_sync(FULL, sid.a, s), bs = __shfl_sync(FULL, sid.b, s), xs_ = __shfl_sync(FULL, sid.x, s);
             if constexpr (MODE == 1) {
                 // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
