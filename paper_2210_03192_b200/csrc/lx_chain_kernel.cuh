@@ -76,6 +76,12 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         }
         __syncthreads();
         const int kmax = *s_kmax;
+        // the finished shell-sets of the previous batch are still in TC (nothing writes TC before the end of the first
+        // pass): the consumer warps, idle while the producers fill the ring, copy them out now
+        if constexpr (MODE == 0) {
+            if (warp < P.ncx && batch != (long long)blockIdx.x)
+                batch_copy_out<CC::NINT, SLOTN>(TC, out, batch - gridDim.x, map.nsets, warp * 32 + lane, P.ncx * 32);
+        }
 
         // ---- passes over the primitive loop: ONE ring runs through all passes (slot g = pass * kmax + q), so the producers
         // of pass i+1 fill it while the consumers of pass i finish; roles are fixed for the batch: warps [0, NCX) consume
@@ -234,7 +240,14 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             }
         }
         __syncthreads();
-        chain_epilogue<LX, LA, LB, MODE, NW>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+        chain_epilogue<LX, LA, LB, MODE, NW, true>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+    }
+    // the last batch of this block (the epilogue ended with a block barrier)
+    if constexpr (MODE == 0) {
+        if ((long long)blockIdx.x < nbatch) {
+            const long long last = blockIdx.x + ((nbatch - 1 - blockIdx.x) / gridDim.x) * gridDim.x;
+            batch_copy_out<CC::NINT, SLOTN>(TC, out, last, map.nsets, tid, NW * 32);
+        }
     }
 }
 

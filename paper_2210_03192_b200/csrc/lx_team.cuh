@@ -235,9 +235,34 @@ __device__ __forceinline__ void target_drop(int ti, const double *__restrict__ a
     });
 }
 
+// a8: a batch is one contiguous run of out[]; `nthr` threads (index tid) copy it, four independent elements in flight each.
+template <int NINT, int SLOTN>
+__device__ __forceinline__ void batch_copy_out(const double *__restrict__ TC, double *__restrict__ out, long long batch,
+                                               long long nsets, int tid, int nthr) {
+    const long long nlive = min((long long)32, nsets - batch * 32);
+    const int total = (int)nlive * NINT;
+    double *o = out + batch * 32 * NINT;
+    for (int it0 = tid; it0 < total; it0 += nthr * 4) {
+        double v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int it = it0 + u * nthr;
+            if (it < total) {
+                const int sset = it / NINT, r = it - sset * NINT;
+                v[u] = TC[(size_t)sset * SLOTN + r];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int it = it0 + u * nthr;
+            if (it < total) o[it] = v[u];
+        }
+    }
+}
+
 // After the targets of a batch were dropped (and a block barrier): gather (e0|c) = U_{0,c} + Σ_{n>0} β(c,n) U_{|n|,c−2n},
 // HRR in registers per (set = lane, c) in place in TC, then one warp per set stores / digests the finished shell-set.
-template <int LX, int LA, int LB, int MODE, int NW>
+template <int LX, int LA, int LB, int MODE, int NW, bool DEFER = false>
 __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const double *__restrict__ UB,
                                                const PartnerTab *__restrict__ pt, int warp, int lane,
                                                long long batch, const SetMap &map, const DevShells &aux,
@@ -304,29 +329,8 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
         }
         __syncthreads();
     }
-    if constexpr (MODE == 0) {
-        // a8: the batch is one contiguous run of out[]; all warps copy it, four independent elements in flight per lane
-        const long long nlive = min((long long)32, map.nsets - batch * 32);
-        const int total = (int)nlive * NINT;
-        double *o = out + batch * 32 * NINT;
-        const int tid = warp * 32 + lane;
-        for (int it0 = tid; it0 < total; it0 += NW * 32 * 4) {
-            double v[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int it = it0 + u * NW * 32;
-                if (it < total) {
-                    const int sset = it / NINT, r = it - sset * NINT;
-                    v[u] = TC[(size_t)sset * SLOTN + r];
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int it = it0 + u * NW * 32;
-                if (it < total) o[it] = v[u];
-            }
-        }
-    }
+    // a8 (DEFER: the caller copies the batch out later, overlapped with the start of the next batch)
+    if constexpr (MODE == 0 && !DEFER) batch_copy_out<NINT, SLOTN>(TC, out, batch, map.nsets, warp * 32 + lane, NW * 32);
     for (int s = warp; MODE != 0 && s < 32; s += NW) {
         const long long sid_s = batch * 32 + s;
         if (sid_s >= map.nsets) break;                    // warp-uniform
