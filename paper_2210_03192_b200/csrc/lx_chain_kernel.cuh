@@ -23,61 +23,70 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]: (e0|c), then the finished shell-set
     double *ZB = TC + (size_t)32 * SLOTN;                    // ring of start-vector buffers
-    double *hd = ZB + (size_t)CC::ZBD;                 // header doubles [9][32]: A, C, AB
-    long long *hpo = reinterpret_cast<long long *>(hd + 9 * 32);
-    int *hi = reinterpret_cast<int *>(hpo + 32);             // [6][32]: xo0, Kab, K, a, b, x
-    int *s_kmax = hi + 6 * 32;
-    PartnerTab *pt = reinterpret_cast<PartnerTab *>(hd + CC::HDRD + 4);
+    double *hd0 = ZB + (size_t)CC::ZBD;                     // two header buffers: [9][32] doubles A, C, AB; po; 6 ints; kmax
+    PartnerTab *pt = reinterpret_cast<PartnerTab *>(hd0 + CC::HDRD + 4);
     if (threadIdx.x == 0) partner_tab_build<LX>(pt);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long nbatch = (map.nsets + 31) / 32;
 
-    for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
-        // ---- set of each lane (warp 0 decodes, everybody reads the header) ---------------------------------------------
-        if (warp == 0) {
-            const long long sid = batch * 32 + lane;
-            const bool live = sid < map.nsets;
-            int p = 0, xs = 0;
-            if (live) {
-                if (map.cum == nullptr) {
-                    p = (int)(sid / map.nx);
-                    xs = (int)(sid - (long long)p * map.nx);
-                } else {
-                    int lo = 0, hi_ = map.npair;             // largest p with cum[p] <= sid
-                    while (hi_ - lo > 1) {
-                        const int mid = (lo + hi_) >> 1;
-                        if (map.cum[mid] <= sid) lo = mid; else hi_ = mid;
-                    }
-                    p = lo;
-                    xs = (int)(sid - map.cum[p]);
+    // header of batch bb into buffer hb (warp 0, lane = set); batches past the end decode as empty sets
+    auto decode_header = [&](long long bb, int hb) {
+        double *hd = hd0 + (size_t)hb * CC::HDR1;
+        long long *hpo = reinterpret_cast<long long *>(hd + 9 * 32);
+        int *hi = reinterpret_cast<int *>(hpo + 32);
+        int *s_kmax = hi + 6 * 32;
+        const long long sid = bb * 32 + lane;
+        const bool live = sid < map.nsets;
+        int p = 0, xs = 0;
+        if (live) {
+            if (map.cum == nullptr) {
+                p = (int)(sid / map.nx);
+                xs = (int)(sid - (long long)p * map.nx);
+            } else {
+                int lo = 0, hi_ = map.npair;             // largest p with cum[p] <= sid
+                while (hi_ - lo > 1) {
+                    const int mid = (lo + hi_) >> 1;
+                    if (map.cum[mid] <= sid) lo = mid; else hi_ = mid;
                 }
+                p = lo;
+                xs = (int)(sid - map.cum[p]);
             }
-            const int a = map.pair_list[2 * p + swapped], b = map.pair_list[2 * p + 1 - swapped];
-            const int x = map.x_list[xs];
-            const int Kab = prim.K[a] * prim.K[b];
-            const int K = live ? Kab * aux.K[x] : 0;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const double Ad = prim.center[3 * a + d];
-                hd[d * 32 + lane] = Ad;
-                hd[(3 + d) * 32 + lane] = aux.center[3 * x + d];
-                hd[(6 + d) * 32 + lane] = Ad - prim.center[3 * b + d];
-            }
-            hpo[lane] = pdat.pd_off ? pdat.pd_off[p] : (long long)p * pdat.kstride;
-            hi[0 * 32 + lane] = aux.prim_off[x];
-            hi[1 * 32 + lane] = Kab;
-            hi[2 * 32 + lane] = K;
-            hi[3 * 32 + lane] = a;
-            hi[4 * 32 + lane] = b;
-            hi[5 * 32 + lane] = x;
-            const int km = __reduce_max_sync(FULL, K);
-            if (lane == 0) *s_kmax = km;
         }
+        const int a = map.pair_list[2 * p + swapped], b = map.pair_list[2 * p + 1 - swapped];
+        const int x = map.x_list[xs];
+        const int Kab = prim.K[a] * prim.K[b];
+        const int K = live ? Kab * aux.K[x] : 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double Ad = prim.center[3 * a + d];
+            hd[d * 32 + lane] = Ad;
+            hd[(3 + d) * 32 + lane] = aux.center[3 * x + d];
+            hd[(6 + d) * 32 + lane] = Ad - prim.center[3 * b + d];
+        }
+        hpo[lane] = pdat.pd_off ? pdat.pd_off[p] : (long long)p * pdat.kstride;
+        hi[0 * 32 + lane] = aux.prim_off[x];
+        hi[1 * 32 + lane] = Kab;
+        hi[2 * 32 + lane] = K;
+        hi[3 * 32 + lane] = a;
+        hi[4 * 32 + lane] = b;
+        hi[5 * 32 + lane] = x;
+        const int km = __reduce_max_sync(FULL, K);
+        if (lane == 0) *s_kmax = km;
+    };
+    if (warp == 0) decode_header(blockIdx.x, 0);
+    int hbuf = 0;
+    for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x, hbuf ^= 1) {
+        const double *hd = hd0 + (size_t)hbuf * CC::HDR1;    // this batch's header (decoded during the previous batch)
+        const long long *hpo = reinterpret_cast<const long long *>(hd + 9 * 32);
+        const int *hi = reinterpret_cast<const int *>(hpo + 32);
+        const int *s_kmax = hi + 6 * 32;
         __syncthreads();
         const int kmax = *s_kmax;
         // the finished shell-sets of the previous batch are still in TC (nothing writes TC before the end of the first
         // pass): the consumer warps, idle while the producers fill the ring, copy them out now
+        // warp 0 decodes the next batch while the producers fill the ring (it is a consumer and would idle)
+        if (warp == 0) decode_header(batch + gridDim.x, hbuf ^ 1);
         if constexpr (MODE == 0) {
             if (warp < P.ncx && batch != (long long)blockIdx.x)
                 batch_copy_out<CC::NINT, SLOTN>(TC, out, batch - gridDim.x, map.nsets, warp * 32 + lane, P.ncx * 32);
