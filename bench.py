@@ -31,7 +31,7 @@ UNIT = "integrals/s"
 WORKLOAD = "configs[1]: 45 classes (Lx 0..4 | La,Lb 0..2), K_total=9, 1024 pairs x 256 aux per class"
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk/SM x 2 x sm_max_mhz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures under profiles/ (class -> bytes)
-NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): 1.072102e9 + 0.955e6}   # profiles/r01_ncu_chain_4_2_2.md
+NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): 1.071891e9 + 0.905e6}   # profiles/r01_ncu_chain_4_2_2.md
 # SURVEY.md §8(d) table, flops per shell-set at K = 9 for the classes it lists
 SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
                         (4, 1, 1): 29322, (4, 2, 2): 111054}
