@@ -142,6 +142,7 @@ def main():
     ap.add_argument("--nx", type=int, default=256, help="aux shells per class (default = config 2)")
     ap.add_argument("--classes", default="", help="profiling aid: restrict the sweep to e.g. '4,2,1;4,0,0' (default: all 45)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--streams", type=int, default=2, help="CUDA streams the classes of a step are spread over")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-df", action="store_true", help="skip the DF-J (config 4) side measurement")
     args = ap.parse_args()
@@ -177,20 +178,60 @@ def main():
                    torch.from_numpy(cfg["x_idx"]).to(dev), torch.from_numpy(cfg["pair_idx"]).to(dev))
     nsets = args.npair * args.nx
     max_int = max(nint_set(c) for c in classes) * nsets
-    out = torch.empty(max_int, dtype=torch.float64, device=dev)
-    ws = torch.empty(lx.lx_eri3_workspace_bytes(0, 0, 0, args.nx, args.npair, 9), dtype=torch.uint8, device=dev)
+    # every class has its own output region and workspace, so that classes may run concurrently on several streams
+    ints_cls = [nint_set(c) * nsets for c in classes]
+    offs = np.concatenate([[0], np.cumsum(ints_cls)])
+    out_all = torch.empty(int(offs[-1]), dtype=torch.float64, device=dev)
+    outs = [out_all[int(offs[i]):int(offs[i + 1])] for i in range(len(classes))]
+    ws_bytes = lx.lx_eri3_workspace_bytes(0, 0, 0, args.nx, args.npair, 9)
+    wss = [torch.empty(ws_bytes, dtype=torch.uint8, device=dev) for _ in classes]
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
     ints_per_step = sum(nint_set(c) for c in classes) * nsets
     probe = lx.lx_fp64_probe(20000)
 
-    def one_step(evs=None):
-        for i, c in enumerate(classes):
-            da, dp, dx, dpr = devs[c]
-            if evs is not None:
-                evs[i][0].record()
-            lx.lx_eri3_batch(c[0], c[1], c[2], da, dp, dx, dpr, out=out, workspace=ws, kmax=9)
-            if evs is not None:
-                evs[i][1].record()
+    def launch(i, stream=None):
+        c = classes[i]
+        da, dp, dx, dpr = devs[c]
+        lx.lx_eri3_batch(c[0], c[1], c[2], da, dp, dx, dpr, out=outs[i], workspace=wss[i], kmax=9, stream=stream)
+
+    def serial_step(evs):
+        """One pass on the current stream with an event pair per class (per-class times for the roofline)."""
+        for i in range(len(classes)):
+            evs[i][0].record()
+            launch(i)
+            evs[i][1].record()
+
+    # The timed step: the independent classes are spread over `--streams` CUDA streams (longest first, each to the least
+    # loaded stream by the cost model), so that the latency-bound small classes run in the shadow of the large ones.
+    main = torch.cuda.current_stream()
+    side = [torch.cuda.Stream(device=dev) for _ in range(max(args.streams, 1) - 1)]
+    cost = [costmodel.flops_per_set(*c, 9) + 8.0 * nint_set(c) + 2000.0 for c in classes]
+    load = [0.0] * (1 + len(side))
+    plan = []
+    for i in sorted(range(len(classes)), key=lambda i: -cost[i]):
+        k = int(np.argmin(load))
+        load[k] += cost[i]
+        plan.append((i, k))
+
+    def one_step():
+        if not side:
+            for i, _ in plan:
+                launch(i)
+            return
+        fork = torch.cuda.Event()
+        fork.record(main)
+        for st in side:
+            st.wait_event(fork)
+        for i, k in plan:
+            if k == 0:
+                launch(i, main)
+            else:
+                with torch.cuda.stream(side[k - 1]):
+                    launch(i, side[k - 1])
+        for st in side:
+            join = torch.cuda.Event()
+            join.record(st)
+            main.wait_event(join)
 
     def barrier():
         if world > 1:
@@ -204,21 +245,27 @@ def main():
     sampler.start()
     launches0 = lx.lx_launch_count()
     step_ms = []
-    class_ms = np.zeros(len(classes))
     for _ in range(args.steps):
         flush.fill_(1)                      # L2 flush between timed iterations (outside the timed interval)
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in classes]
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         s0.record()
-        one_step(evs)
+        one_step()
         s1.record()
         barrier()
         step_ms.append(s0.elapsed_time(s1))
-        class_ms += np.array([a.elapsed_time(b) for a, b in evs])
     launches = lx.lx_launch_count() - launches0
     clocks = sampler.stop()
-    class_ms /= args.steps
+    # per-class kernel times (roofline of the dominant kernel): three serial passes outside the timed region
+    class_ms = np.zeros(len(classes))
+    for _ in range(3):
+        flush.fill_(1)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in classes]
+        barrier()
+        serial_step(evs)
+        barrier()
+        class_ms += np.array([a.elapsed_time(b) for a, b in evs]) / 3
+    serial_ms = float(class_ms.sum())
     t_total = torch.tensor([sum(step_ms) * 1e-3], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
@@ -316,7 +363,9 @@ def main():
                            "shell_sets_per_step": nsets * len(classes) * world, "integrals_per_step": ints_per_step * world,
                            "l2": "flushed between timed steps (256 MiB fill, outside the timed interval); each step also writes "
                                  f"{ints_per_step * 8 / 1e9:.1f} GB of output",
-                           "parallelism": f"{world} x independent batch (no collective)"},
+                           "parallelism": f"{world} x independent batch (no collective)",
+                           "streams": f"{1 + len(side)} CUDA streams per step (independent classes overlap); the same classes launched "
+                                      f"back to back on one stream take {serial_ms:.2f} ms (sum of per-class event times)"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
                 "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df,
                 "integrals_per_s_per_class": per_class}
