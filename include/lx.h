@@ -137,8 +137,10 @@ int lx_boys(const double *T, int n, int mmax, double *out, void *stream);
  * 5 timed launches.  This is the measured denominator of the FP64-pipe roofline; synchronises. */
 int lx_fp64_probe(int iters, double *tflops_host);
 
-/* Which kernel template serves a class: "lane" (register-resident, lx_lane.cuh) or "group" (shared-memory,
- * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only. */
+/* Which kernel template serves a class: "team" (register-only chain form, lx_team.cuh), "chain" (warp-specialised
+ * chain form, lx_chain_kernel.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
+ * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only.  The environment
+ * variable LX_FAMILY=team|chain|lane (read once) forces the named family where a class has it: a tuning aid. */
 const char *lx_kernel_family(int lx, int la, int lb);
 
 /* Number of kernel launches the library has issued since lx_init (for the bench's `gpu_launches` claim). */

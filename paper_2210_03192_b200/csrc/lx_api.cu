@@ -160,7 +160,7 @@ using namespace lx;
 // ================================================================================================ C ABI
 extern "C" {
 
-const char *lx_version(void) { return "lx3 0.1 sm_100a (coop kernels, Lx<=6, La,Lb<=4)"; }
+const char *lx_version(void) { return "lx3 0.2 sm_100a (team/chain/lane/group kernels, Lx<=6, La,Lb<=4)"; }
 
 const char *lx_kernel_family(int lx_, int la, int lb) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
