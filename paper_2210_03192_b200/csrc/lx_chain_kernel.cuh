@@ -3,8 +3,10 @@
 #pragma once
 #include "lx_team.cuh"
 
+// 1: classes with three or more passes re-align producers and consumers at every pass boundary (tuning aid; measured
+// within 1 % of the free-running ring, which is the default)
 #ifndef LX_CHAIN_REALIGN
-#define LX_CHAIN_REALIGN 1
+#define LX_CHAIN_REALIGN 0
 #endif
 
 namespace lx {
@@ -97,9 +99,6 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         // (warp w holds target T0 + w of the current pass, or idles through the barriers), warps [NCX, NCX + NPX) produce.
         constexpr int NCX = P.ncx, NPX = P.npx, NBUF = NPX + 1, ZREC = P.zrec;
         constexpr int BCOUNT = (NCX + 1) * 32;               // threads on a full[] / empty[] barrier
-        // measured: with three or more passes the producers running ahead into the code of the next pass cost more
-        // (instruction cache) than the pipeline refill they save, so those classes re-align at every pass boundary
-        // (CONT = npass <= 2)
         const int gtot = P.npass * kmax;                     // ring slots of the batch
         if (warp >= NCX) {
             // ================= producers: ring slots g = j, j + NPX, ... ======================================================
