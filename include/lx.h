@@ -137,6 +137,19 @@ int lx_boys(const double *T, int n, int mmax, double *out, void *stream);
  * 5 timed launches.  This is the measured denominator of the FP64-pipe roofline; synchronises. */
 int lx_fp64_probe(int iters, double *tflops_host);
 
+/* Row a6 of the path (HGPA step 5): Cartesian -> real solid-harmonic transform of the
+ * auxiliary index of finished shell-sets,
+ *     out[set][m][r] = sum_c S_l[m][c] in[set][c][r],   set < nsets, m = 0..2l, c < nc(l), r < nab,
+ * i.e. `in` is the output of lx_eri3_batch viewed as [npair*nx][nc(lx)][nc(la)*nc(lb)] and `out` holds (X_m|ab) for the
+ * pure functions S_lm, m = -l..l in this order (reading G1: the paper's aux functions are solid harmonics).  S_lm are the
+ * real solid harmonics in Racah normalisation (S_l0 = r^l P_l(cos theta); S_20 = z^2 - x^2/2 - y^2/2), each a linear
+ * combination of the Cartesian components of degree l (ABI order, reading G2).  Device pointers, `in != out`, the caller
+ * owns both; asynchronous on `stream`.  LX_EUNSUPPORTED for l > LX_MAX_L_AUX, LX_EINVAL for null / aliased buffers. */
+int lx_cart_to_pure(int lx, int64_t nsets, int nab, const double *in, double *out, void *stream);
+
+/* The matrix S_l used by lx_cart_to_pure, (2l+1) x nc(l) row-major, into HOST memory (no device needed). */
+int lx_solid_matrix(int l, double *matrix_host);
+
 /* Which kernel template serves a class: "team" (register-only chain form, lx_team.cuh), "chain" (warp-specialised
  * chain form, lx_chain_kernel.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
  * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only.  The environment

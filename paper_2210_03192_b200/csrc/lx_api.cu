@@ -22,6 +22,7 @@ struct State {
     int device = -1;
     int num_sms = 0;
     double *boys_tab = nullptr;      // [BOYS_NGRID][BOYS_MROWS]
+    double *solid[LX_MAX_L_AUX + 1] = {};   // per l: (2l+1) x nc(l) Cartesian -> real solid harmonic matrix
     std::atomic<long long> launches{0};
     char cuda_msg[256] = "no CUDA error recorded";
     // grow-only device arena for the host-buffer convenience path
@@ -127,6 +128,88 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double seed,
     if (r == 123.456) sink[0] = r;
 }
 
+// ------------------------------------------------------------------------------------------------ solid harmonics (a6)
+// Real solid harmonics S_lm as polynomials in (x, y, z), Racah normalisation, by the recurrences of the regular solid
+// harmonics (Helgaker, Jorgensen, Olsen, "Molecular Electronic-Structure Theory", eqs. 6.4.70-6.4.73):
+//   S_00 = 1
+//   S_{l+1, l+1}  = sqrt(2^{d_l0} (2l+1)/(2l+2)) (x S_ll - (1 - d_l0) y S_{l,-l})
+//   S_{l+1,-l-1}  = sqrt(2^{d_l0} (2l+1)/(2l+2)) (y S_ll + (1 - d_l0) x S_{l,-l})
+//   S_{l+1, m}    = ((2l+1) z S_lm - sqrt((l+m)(l-m)) r^2 S_{l-1,m}) / sqrt((l+m+1)(l-m+1)),  |m| <= l
+// Row m + l of the matrix holds the coefficients of S_lm over the Cartesian components in ABI order (reading G2).
+// Written for this library; the test oracle uses the closed formula instead and shares nothing with this.
+struct SolidPoly {
+    double c[LX_MAX_L_AUX + 1][LX_MAX_L_AUX + 1][LX_MAX_L_AUX + 1];
+    SolidPoly() { std::memset(c, 0, sizeof(c)); }
+};
+static void poly_axpy_shift(SolidPoly &dst, double f, const SolidPoly &src, int sx, int sy, int sz) {
+    const int N = LX_MAX_L_AUX + 1;
+    for (int x = 0; x + sx < N; ++x)
+        for (int y = 0; y + sy < N; ++y)
+            for (int z = 0; z + sz < N; ++z) dst.c[x + sx][y + sy][z + sz] += f * src.c[x][y][z];
+}
+static void solid_matrices_host(std::vector<std::vector<double>> &mats) {
+    const int LM = LX_MAX_L_AUX;
+    // S[l][m + l]
+    std::vector<std::vector<SolidPoly>> S(LM + 1);
+    S[0].resize(1);
+    S[0][0].c[0][0][0] = 1.0;
+    for (int l = 0; l < LM; ++l) {
+        S[l + 1].resize(2 * l + 3);
+        const double d0 = l == 0 ? 1.0 : 0.0;
+        const double f = std::sqrt(std::pow(2.0, d0) * (2.0 * l + 1.0) / (2.0 * l + 2.0));
+        const SolidPoly &pll = S[l][2 * l], &pml = S[l][0];          // S_{l,l}, S_{l,-l}
+        SolidPoly &top = S[l + 1][2 * l + 2], &bot = S[l + 1][0];    // S_{l+1,l+1}, S_{l+1,-l-1}
+        poly_axpy_shift(top, f, pll, 1, 0, 0);
+        poly_axpy_shift(bot, f, pll, 0, 1, 0);
+        if (l > 0) {
+            poly_axpy_shift(top, -f, pml, 0, 1, 0);
+            poly_axpy_shift(bot, f, pml, 1, 0, 0);
+        }
+        for (int m = -l; m <= l; ++m) {
+            SolidPoly &t = S[l + 1][m + l + 1];
+            const double den = std::sqrt((double)(l + m + 1) * (double)(l - m + 1));
+            poly_axpy_shift(t, (2.0 * l + 1.0) / den, S[l][m + l], 0, 0, 1);
+            if (l >= 1 && std::abs(m) <= l - 1) {
+                const double g2 = -std::sqrt((double)(l + m) * (double)(l - m)) / den;
+                const SolidPoly &q = S[l - 1][m + l - 1];
+                poly_axpy_shift(t, g2, q, 2, 0, 0);
+                poly_axpy_shift(t, g2, q, 0, 2, 0);
+                poly_axpy_shift(t, g2, q, 0, 0, 2);
+            }
+        }
+    }
+    mats.assign(LM + 1, {});
+    for (int l = 0; l <= LM; ++l) {
+        mats[l].assign((size_t)(2 * l + 1) * nc(l), 0.0);
+        for (int m = 0; m < 2 * l + 1; ++m) {
+            int ci = 0;
+            for (int x = l; x >= 0; --x)
+                for (int y = l - x; y >= 0; --y, ++ci) mats[l][(size_t)m * nc(l) + ci] = S[l][m].c[x][y][l - x - y];
+        }
+    }
+}
+
+// out[set][m][r] = sum_c S[m][c] in[set][c][r]; one thread per (set, r), the matrix in shared memory
+__global__ void cart_to_pure_kernel(const double *__restrict__ S, int l, long long nsets, int nab,
+                                    const double *__restrict__ in, double *__restrict__ out) {
+    extern __shared__ double sm[];
+    const int ncl = nc(l), npl = 2 * l + 1;
+    for (int i = threadIdx.x; i < ncl * npl; i += blockDim.x) sm[i] = S[i];
+    __syncthreads();
+    const long long total = nsets * nab;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long set = t / nab;
+        const int r = (int)(t - set * nab);
+        const double *src = in + set * ncl * nab + r;
+        double *dst = out + set * npl * nab + r;
+        for (int m = 0; m < npl; ++m) {
+            double acc = 0.0;
+            for (int c = 0; c < ncl; ++c) acc = fma(sm[m * ncl + c], src[(size_t)c * nab], acc);
+            dst[(size_t)m * nab] = acc;
+        }
+    }
+}
+
 static int check_shells(const lx_shells_t *s, bool need_bf) {
     if (!s) return LX_EINVAL;
     if (s->nshell < 0) return LX_EINVAL;
@@ -198,6 +281,13 @@ int lx_init(int device) {
     if (g.boys_tab) cudaFree(g.boys_tab);
     LX_CUDA(cudaMalloc(&g.boys_tab, tab.size() * sizeof(double)));
     LX_CUDA(cudaMemcpy(g.boys_tab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    std::vector<std::vector<double>> mats;
+    solid_matrices_host(mats);
+    for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
+        if (g.solid[l]) cudaFree(g.solid[l]);
+        LX_CUDA(cudaMalloc(&g.solid[l], mats[l].size() * sizeof(double)));
+        LX_CUDA(cudaMemcpy(g.solid[l], mats[l].data(), mats[l].size() * sizeof(double), cudaMemcpyHostToDevice));
+    }
     g.device = device;
     g.ready = true;
     return LX_OK;
@@ -208,6 +298,10 @@ int lx_finalize(void) {
     if (g.boys_tab) cudaFree(g.boys_tab);
     if (g.arena) cudaFree(g.arena);
     if (g.pinned) cudaFreeHost(g.pinned);
+    for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
+        if (g.solid[l]) cudaFree(g.solid[l]);
+        g.solid[l] = nullptr;
+    }
     g.boys_tab = nullptr;
     g.arena = nullptr;
     g.arena_bytes = 0;
@@ -245,6 +339,31 @@ int lx_fp64_probe(int iters, double *tflops_host) {
     cudaEventDestroy(e1);
     cudaFree(sink);
     *tflops_host = best;
+    return LX_OK;
+}
+
+int lx_solid_matrix(int l, double *matrix_host) {
+    if (l < 0 || l > LX_MAX_L_AUX || !matrix_host) return LX_EINVAL;
+    std::vector<std::vector<double>> mats;
+    solid_matrices_host(mats);
+    std::memcpy(matrix_host, mats[l].data(), mats[l].size() * sizeof(double));
+    return LX_OK;
+}
+
+int lx_cart_to_pure(int lx_, int64_t nsets, int nab, const double *in, double *out, void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (lx_ < 0 || lx_ > LX_MAX_L_AUX) return LX_EUNSUPPORTED;
+    if (nsets < 0 || nab < 0) return LX_EINVAL;
+    if (nsets == 0 || nab == 0) return LX_OK;
+    if (!in || !out || in == out) return LX_EINVAL;
+    const long long total = (long long)nsets * nab;
+    const int threads = 256;
+    long long blocks = (total + threads - 1) / threads;
+    if (blocks > (long long)g.num_sms * 16) blocks = (long long)g.num_sms * 16;
+    const size_t smem = (size_t)(2 * lx_ + 1) * nc(lx_) * sizeof(double);
+    cart_to_pure_kernel<<<(unsigned)blocks, threads, smem, (cudaStream_t)stream>>>(g.solid[lx_], lx_, nsets, nab, in, out);
+    g.launches++;
+    LX_CUDA(cudaGetLastError());
     return LX_OK;
 }
 

@@ -22,7 +22,8 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
-           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family"]
+           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family",
+           "lx_cart_to_pure", "lx_solid_matrix"]
 
 
 class lx_shells_t(C.Structure):
@@ -42,6 +43,8 @@ _lib.lx_schedule_num_sets.argtypes = [C.c_void_p]
 _lib.lx_schedule_num_integrals.restype = C.c_int64
 _lib.lx_schedule_num_integrals.argtypes = [C.c_void_p]
 _lib.lx_schedule_destroy.argtypes = [C.c_void_p]
+_lib.lx_cart_to_pure.argtypes = [C.c_int, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.lx_solid_matrix.argtypes = [C.c_int, C.c_void_p]
 _lib.lx_launch_count.restype = C.c_int64
 _lib.lx_eri3_batch.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(lx_shells_t), C.POINTER(lx_shells_t),
                                C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -246,6 +249,25 @@ def lx_df_J(sched, aux, prim, d, J=None, workspace=None, stream=None):
     _check(_lib.lx_df_J(sched.handle, C.byref(aux.struct), C.byref(prim.struct), d.data_ptr(), J.data_ptr(),
                         J.stride(0), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
     return J
+
+
+def lx_cart_to_pure(lx, cart, out=None, stream=None):
+    """Cartesian → real solid-harmonic transform of the aux index: cart[npair, nx, nc(lx), na, nb] (device) →
+    [npair, nx, 2lx+1, na, nb]."""
+    assert cart.dtype == torch.float64 and cart.is_cuda and cart.is_contiguous() and cart.dim() == 5
+    npair, nx, ncx, na, nb = cart.shape
+    assert ncx == ncart(lx)
+    if out is None:
+        out = torch.empty((npair, nx, 2 * lx + 1, na, nb), dtype=torch.float64, device=cart.device)
+    _check(_lib.lx_cart_to_pure(lx, C.c_int64(npair * nx), na * nb, cart.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def lx_solid_matrix(l):
+    """The (2l+1) × nc(l) matrix lx_cart_to_pure applies (host; needs no device)."""
+    m = np.zeros((2 * l + 1, ncart(l)), dtype=np.float64)
+    _check(_lib.lx_solid_matrix(l, m.ctypes.data))
+    return m
 
 
 def lx_boys(T, mmax, stream=None):

@@ -73,3 +73,16 @@ def test_shard_pairs_partition():
                 assert tot.max() - tot.min() <= cost.max() * 1.0001 + 1e-9
     with pytest.raises(ValueError):
         shard.shard_pairs(pairs, 2, 2)
+
+
+def test_solid_matrix_matches_oracle(lx):
+    """Row a6: the library builds its Cartesian -> solid-harmonic matrices by the recurrences of the regular solid
+    harmonics, the oracle by the closed formula; the two independent routes must agree for every l (host only)."""
+    from oracle import solid
+    for l in range(7):
+        got = lx.lx_solid_matrix(l)
+        ref = solid.solid_matrix(l)
+        assert got.shape == ref.shape == (2 * l + 1, (l + 1) * (l + 2) // 2)
+        assert np.max(np.abs(got - ref)) <= 1e-13 * np.max(np.abs(ref)), l
+    with pytest.raises(lx.LxError):
+        lx.lx_solid_matrix(7)

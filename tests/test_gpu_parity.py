@@ -239,3 +239,22 @@ def test_store_mode_is_deterministic(lx, cls):
     a = _run(lx, cfg)
     for _ in range(3):
         assert np.array_equal(a, _run(lx, cfg))
+
+
+@pytest.mark.parametrize("cls", [(2, 1, 1), (4, 2, 2), (3, 2, 0), (6, 1, 0), (1, 0, 0), (5, 2, 1)])
+def test_cart_to_pure_transform(lx, oracle, cls):
+    """Row a6 (HGPA step 5): (X_m|ab) for solid-harmonic aux functions = lx_cart_to_pure applied to the
+    Cartesian shell-sets, against the oracle's Cartesian integrals x the oracle's own solid-harmonic matrix."""
+    import torch
+    from oracle import solid
+    lxa, la, lb = cls
+    cfg = gen.config2(lxa, la, lb, npair=23, nx=17) if lxa <= 4 else gen.config3(lxa, la, lb, kprim=2, npair=9, nx=5)
+    aux, prim = lx.DeviceShells(cfg["aux"]), lx.DeviceShells(cfg["prim"])
+    cart = lx.lx_eri3_batch(lxa, la, lb, aux, prim, cfg["x_idx"], cfg["pair_idx"])
+    got = lx.lx_cart_to_pure(lxa, cart)
+    torch.cuda.synchronize()
+    ref = solid.cart_to_pure(lxa, oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"]))
+    assert got.shape == ref.shape
+    _check(got.cpu().numpy(), ref)
+    with pytest.raises(lx.LxError):                                   # in == out is refused
+        lx._check(lx._lib.lx_cart_to_pure(lxa, 1, 1, cart.data_ptr(), cart.data_ptr(), None))
