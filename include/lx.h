@@ -147,6 +147,18 @@ int lx_fp64_probe(int iters, double *tflops_host);
  * owns both; asynchronous on `stream`.  LX_EUNSUPPORTED for l > LX_MAX_L_AUX, LX_EINVAL for null / aliased buffers. */
 int lx_cart_to_pure(int lx, int64_t nsets, int nab, const double *in, double *out, void *stream);
 
+/* (X_m|ab) for SOLID-HARMONIC auxiliary functions (the paper's own target (ab|c); SURVEY.md §8(f)
+ * NEXT-1): same arguments as lx_eri3_batch plus kmax_pair (largest K_a*K_b of the listed pairs), and
+ *     out[npair][nx][2lx+1][nc(la)][nc(lb)],  m = -lx..lx.
+ * Classes served by the team kernel with lx >= 2 run fused: for a pure ket eq. 2 is exact after
+ * projection, so only the level-0 chain targets are evaluated and the solid-harmonic matrix is applied in the epilogue.
+ * Other classes evaluate the Cartesian shell-sets into the workspace and apply lx_cart_to_pure.  The workspace must hold
+ * lx_eri3_pure_workspace_bytes(...) bytes (LX_ENOMEM otherwise); everything else as for lx_eri3_batch. */
+int lx_eri3_batch_pure(int lx, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim, const int32_t *x_idx,
+                       int nx, const int32_t *pair_idx, int npair, int kmax_pair, double *out, void *workspace,
+                       size_t workspace_bytes, void *stream);
+size_t lx_eri3_pure_workspace_bytes(int lx, int la, int lb, int nx, int npair, int kmax_pair);
+
 /* The matrix S_l used by lx_cart_to_pure, (2l+1) x nc(l) row-major, into HOST memory (no device needed). */
 int lx_solid_matrix(int l, double *matrix_host);
 

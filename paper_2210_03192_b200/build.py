@@ -18,7 +18,7 @@ EXTRA = os.environ.get("LX_EXTRA_NVCC", "").split()
 NVCC_FLAGS += EXTRA
 
 LX_RANGE = range(7)      # aux angular momentum 0..LX_MAX_L_AUX
-MODES = range(3)         # 0 store, 1 gamma, 2 J
+MODES = range(4)         # 0 store, 1 gamma, 2 J, 3 store with solid-harmonic aux functions
 
 
 def _headers():

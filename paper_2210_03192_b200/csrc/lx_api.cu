@@ -44,10 +44,11 @@ static int cuda_fail(cudaError_t e) {
         if (_e != cudaSuccess) return cuda_fail(_e);  \
     } while (0)
 
-static const launch_fn k_launch[3][7] = {
+static const launch_fn k_launch[4][7] = {
     {launch_lx0_mode0, launch_lx1_mode0, launch_lx2_mode0, launch_lx3_mode0, launch_lx4_mode0, launch_lx5_mode0, launch_lx6_mode0},
     {launch_lx0_mode1, launch_lx1_mode1, launch_lx2_mode1, launch_lx3_mode1, launch_lx4_mode1, launch_lx5_mode1, launch_lx6_mode1},
     {launch_lx0_mode2, launch_lx1_mode2, launch_lx2_mode2, launch_lx3_mode2, launch_lx4_mode2, launch_lx5_mode2, launch_lx6_mode2},
+    {launch_lx0_mode3, launch_lx1_mode3, launch_lx2_mode3, launch_lx3_mode3, launch_lx4_mode3, launch_lx5_mode3, launch_lx6_mode3},
 };
 
 // ------------------------------------------------------------------------------------------------ Boys table (host)
@@ -189,11 +190,13 @@ static void solid_matrices_host(std::vector<std::vector<double>> &mats) {
     }
 }
 
-// out[set][m][r] = sum_c S[m][c] in[set][c][r]; one thread per (set, r), the matrix in shared memory
-__global__ void cart_to_pure_kernel(const double *__restrict__ S, int l, long long nsets, int nab,
-                                    const double *__restrict__ in, double *__restrict__ out) {
-    extern __shared__ double sm[];
-    const int ncl = nc(l), npl = 2 * l + 1;
+// out[set][m][r] = sum_c S[m][c] in[set][c][r]; one thread per (set, r): the nc(l) inputs are read once into
+// registers (coalesced over r), the matrix sits in shared memory; HBM-bound (reads nc(l), writes 2l+1 doubles per thread)
+template <int L>
+__global__ void __launch_bounds__(256) cart_to_pure_kernel(const double *__restrict__ S, long long nsets, int nab,
+                                                           const double *__restrict__ in, double *__restrict__ out) {
+    constexpr int ncl = nc(L), npl = 2 * L + 1;
+    __shared__ double sm[ncl * npl];
     for (int i = threadIdx.x; i < ncl * npl; i += blockDim.x) sm[i] = S[i];
     __syncthreads();
     const long long total = nsets * nab;
@@ -202,9 +205,14 @@ __global__ void cart_to_pure_kernel(const double *__restrict__ S, int l, long lo
         const int r = (int)(t - set * nab);
         const double *src = in + set * ncl * nab + r;
         double *dst = out + set * npl * nab + r;
+        double v[ncl];
+#pragma unroll
+        for (int c = 0; c < ncl; ++c) v[c] = __ldg(src + (size_t)c * nab);
+#pragma unroll
         for (int m = 0; m < npl; ++m) {
             double acc = 0.0;
-            for (int c = 0; c < ncl; ++c) acc = fma(sm[m * ncl + c], src[(size_t)c * nab], acc);
+#pragma unroll
+            for (int c = 0; c < ncl; ++c) acc = fma(sm[m * ncl + c], v[c], acc);
             dst[(size_t)m * nab] = acc;
         }
     }
@@ -360,8 +368,12 @@ int lx_cart_to_pure(int lx_, int64_t nsets, int nab, const double *in, double *o
     const int threads = 256;
     long long blocks = (total + threads - 1) / threads;
     if (blocks > (long long)g.num_sms * 16) blocks = (long long)g.num_sms * 16;
-    const size_t smem = (size_t)(2 * lx_ + 1) * nc(lx_) * sizeof(double);
-    cart_to_pure_kernel<<<(unsigned)blocks, threads, smem, (cudaStream_t)stream>>>(g.solid[lx_], lx_, nsets, nab, in, out);
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (lx_) {
+#define LX_C2P(LV) case LV: cart_to_pure_kernel<LV><<<(unsigned)blocks, threads, 0, st>>>(g.solid[LV], nsets, nab, in, out); break;
+        LX_C2P(0) LX_C2P(1) LX_C2P(2) LX_C2P(3) LX_C2P(4) LX_C2P(5) LX_C2P(6)
+#undef LX_C2P
+    }
     g.launches++;
     LX_CUDA(cudaGetLastError());
     return LX_OK;
@@ -416,6 +428,51 @@ int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shel
     g.launches++;
     if (e != cudaSuccess) return cuda_fail(e);
     return LX_OK;
+}
+
+size_t lx_eri3_pure_workspace_bytes(int lx_, int la, int lb, int nx, int npair, int kmax_pair) {
+    // pair data + (for classes without a fused kernel) the Cartesian shell-sets the transform reads
+    const size_t base = lx_eri3_workspace_bytes(lx_, la, lb, nx, npair, kmax_pair);
+    if (npair <= 0 || nx <= 0 || !class_supported(lx_, la, lb)) return base;
+    return base + 256 + (size_t)npair * nx * nc(lx_) * nc(la) * nc(lb) * sizeof(double);
+}
+
+int lx_eri3_batch_pure(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim, const int32_t *x_idx,
+                       int nx, const int32_t *pair_idx, int npair, int kmax_pair, double *out, void *workspace,
+                       size_t workspace_bytes, void *stream) {
+    if (!g.ready) return LX_ENOTINIT;
+    if (nx < 0 || npair < 0 || kmax_pair < 0) return LX_EINVAL;
+    if (!class_supported(lx_, la, lb)) return LX_EUNSUPPORTED;
+    if (nx == 0 || npair == 0) return LX_OK;
+    int rc;
+    if ((rc = check_shells(aux, false)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, false)) != LX_OK) return rc;
+    if (!x_idx || !pair_idx || !out || !workspace || kmax_pair < 1) return LX_EINVAL;
+    const size_t pd_bytes = lx_eri3_workspace_bytes(lx_, la, lb, nx, npair, kmax_pair);
+    if (workspace_bytes < pd_bytes) return LX_ENOMEM;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int swapped = la < lb ? 1 : 0;
+    const int cla = swapped ? lb : la, clb = swapped ? la : lb;
+    DevShells dprim = dev_view(prim), daux = dev_view(aux);
+    double *pd = reinterpret_cast<double *>(workspace);
+    // fused path: level-0 chain targets + solid-harmonic projection in the epilogue (team kernel classes, Lx >= 2)
+    if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kmax_pair, pd, st)) != LX_OK) return rc;
+    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr};
+    PairData pdat{pd, nullptr, kmax_pair};
+    DfArgs df{g.solid[lx_], nullptr, 0};
+    cudaError_t e = k_launch[3][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
+    if (e == cudaSuccess) {
+        g.launches++;
+        return LX_OK;
+    }
+    if (e != cudaErrorNotSupported) return cuda_fail(e);
+    // fallback: Cartesian shell-sets into the workspace, then row a6 as its own kernel
+    const size_t cart_bytes = (size_t)npair * nx * nc(lx_) * nc(la) * nc(lb) * sizeof(double);
+    const size_t coff = (pd_bytes + 255) & ~(size_t)255;
+    if (workspace_bytes < coff + cart_bytes) return LX_ENOMEM;
+    double *cart = reinterpret_cast<double *>(reinterpret_cast<char *>(workspace) + coff);
+    if ((rc = lx_eri3_batch(lx_, la, lb, aux, prim, x_idx, nx, pair_idx, npair, cart, workspace, pd_bytes, stream)) != LX_OK) return rc;
+    return lx_cart_to_pure(lx_, (int64_t)npair * nx, nc(la) * nc(lb), cart, out, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ schedule (a0)

@@ -9,7 +9,7 @@ namespace lx {
                                              const DevShells &prim, const PairData &pdat, const double *boys_tab, \
                                              double *out, int swapped, const DfArgs &df, int num_sms,             \
                                              cudaStream_t stream);
-#define LX_DECL3(LXV) LX_DECL(LXV, 0) LX_DECL(LXV, 1) LX_DECL(LXV, 2)
+#define LX_DECL3(LXV) LX_DECL(LXV, 0) LX_DECL(LXV, 1) LX_DECL(LXV, 2) LX_DECL(LXV, 3)
 LX_DECL3(0) LX_DECL3(1) LX_DECL3(2) LX_DECL3(3) LX_DECL3(4) LX_DECL3(5) LX_DECL3(6)
 #undef LX_DECL3
 #undef LX_DECL

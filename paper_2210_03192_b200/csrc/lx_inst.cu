@@ -8,7 +8,7 @@
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
-#error "compile with -DINST_LX=<0..6> -DINST_MODE=<0..2>"
+#error "compile with -DINST_LX=<0..6> -DINST_MODE=<0..3>"
 #endif
 
 namespace lx {
@@ -42,6 +42,13 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
     // measured (B200): for Lx <= 4 the team kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets;
     // for Lx = 5, 6 it beats the lane kernel while at most three warps hold the targets
     constexpr bool has_team = TW > 0 && (LX <= 4 ? (LA + LB <= 2 || TW <= (wide ? 3 : LX_TEAM_WMAX)) : (LA + LB >= 1 && TW <= 3)), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
+    if constexpr (MODE == 3) {
+        // fused solid-harmonic aux functions: team kernel only; the caller falls back to Cartesian + lx_cart_to_pure
+        if constexpr (has_team && LX >= 2)
+            return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+        else
+            return cudaErrorNotSupported;
+    } else {
     const int ov = family_override();
     if constexpr (has_team) {
         if (ov == 0 || ov == 1 || (ov == 2 && !has_chain) || (ov == 3 && !has_lane))
@@ -55,6 +62,7 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    }
 }
 
 #define LX_CASE(LA_, LB_)                                                                                        \

@@ -235,6 +235,44 @@ __device__ __forceinline__ void target_drop(int ti, const double *__restrict__ a
     });
 }
 
+// a7: HRR (eq. 1) of one (set, ket component) in registers: H0 = (e0| for the shells e = LA..LA+LB in,
+// (a b| out to reg[a][b] (tr: reg[b][a], the caller's order of a mirrored class).  Written for LB <= 2.
+template <int LA, int LB>
+__device__ __forceinline__ void hrr_store(const double (&H0)[off(LA + LB + 1) - off(LA)], const double (&AB)[3],
+                                          double *__restrict__ reg, bool tr) {
+    constexpr int E = LA + LB, NACC = off(E + 1) - off(LA), NA = nc(LA);
+    if constexpr (LB == 0) {
+        static_for<0, NACC>([&](auto ii) { reg[decltype(ii)::value] = H0[decltype(ii)::value]; });
+    } else {
+        constexpr int NA1 = off(E) - off(LA);        // bra components of the shells LA..E−1
+        double H1[NA1 * 3];
+        static_for<0, NA1>([&](auto ial) {
+            constexpr int al = decltype(ial)::value, g = off(LA) + al;
+            static_for<0, 3>([&](auto id) {
+                constexpr int d = decltype(id)::value;
+                H1[al * 3 + d] = fma(AB[d], H0[al], H0[cart_up(g, d) - off(LA)]);
+            });
+        });
+        if constexpr (LB == 1) {
+            static_for<0, NA * 3>([&](auto ii) {
+                constexpr int i = decltype(ii)::value;
+                reg[tr ? (i % 3) * NA + i / 3 : i] = H1[i];
+            });
+        } else {
+            static_assert(LB <= 2, "HRR written for Lb <= 2");
+            static_for<0, NA>([&](auto ial) {
+                constexpr int al = decltype(ial)::value, g = off(LA) + al;
+                static_for<0, 6>([&](auto ib) {
+                    constexpr int bj = decltype(ib)::value, gb = off(2) + bj;
+                    constexpr int d = (int)(cart_entry(gb) >> 24);
+                    constexpr int b1 = cart_dn(gb, d) - off(1);
+                    reg[tr ? bj * NA + al : al * 6 + bj] = fma(AB[d], H1[al * 3 + b1], H1[(cart_up(g, d) - off(LA)) * 3 + b1]);
+                });
+            });
+        }
+    }
+}
+
 // a8: a batch is one contiguous run of out[]; `nthr` threads (index tid) copy it, four independent elements in flight each.
 template <int NINT, int SLOTN>
 __device__ __forceinline__ void batch_copy_out(const double *__restrict__ TC, double *__restrict__ out, long long batch,
@@ -295,36 +333,7 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
                         });
                     }
                 }
-                if constexpr (LB == 0) {
-                    static_for<0, NACC>([&](auto ii) { reg[decltype(ii)::value] = H0[decltype(ii)::value]; });
-                } else {
-                    constexpr int NA1 = off(E) - off(LA);        // bra components of the shells LA..E−1
-                    double H1[NA1 * 3];
-                    static_for<0, NA1>([&](auto ial) {
-                        constexpr int al = decltype(ial)::value, g = off(LA) + al;
-                        static_for<0, 3>([&](auto id) {
-                            constexpr int d = decltype(id)::value;
-                            H1[al * 3 + d] = fma(AB[d], H0[al], H0[cart_up(g, d) - off(LA)]);
-                        });
-                    });
-                    if constexpr (LB == 1) {
-                        static_for<0, NA * 3>([&](auto ii) {
-                            constexpr int i = decltype(ii)::value;
-                            reg[tr ? (i % 3) * NA + i / 3 : i] = H1[i];
-                        });
-                    } else {
-                        static_assert(LB <= 2, "chain epilogue: HRR written for Lb <= 2");
-                        static_for<0, NA>([&](auto ial) {
-                            constexpr int al = decltype(ial)::value, g = off(LA) + al;
-                            static_for<0, 6>([&](auto ib) {
-                                constexpr int bj = decltype(ib)::value, gb = off(2) + bj;
-                                constexpr int d = (int)(cart_entry(gb) >> 24);
-                                constexpr int b1 = cart_dn(gb, d) - off(1);
-                                reg[tr ? bj * NA + al : al * 6 + bj] = fma(AB[d], H1[al * 3 + b1], H1[(cart_up(g, d) - off(LA)) * 3 + b1]);
-                            });
-                        });
-                    }
-                }
+                hrr_store<LA, LB>(H0, AB, reg, tr);
             }
         }
         __syncthreads();
@@ -368,6 +377,41 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
 }
 
 
+// MODE 3 — solid-harmonic aux functions, fused (HGPA step 5).  For a pure ket the
+// two-term relation eq. 2 is exact after projection: only the level-0 targets G_c = (Π B^c Z^{(Lx)}) are
+// evaluated, and (X_m|e0) = Σ_c S_l[m][c] G_c with the real solid harmonics S_lm (lx.h, lx_cart_to_pure).  Per (set = lane,
+// m): transform, HRR in registers, store into the pure region PR [set][m][a][b]; then the batch leaves coalesced.
+template <int LX, int LA, int LB, int NW>
+__device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, double *__restrict__ PR,
+                                              const double *__restrict__ smat, int warp, int lane, long long batch,
+                                              const SetMap &map, const DevShells &prim, double *__restrict__ out, int swapped) {
+    using CC = ChainCls<LX, LA, LB>;
+    constexpr int NACC = CC::NACC, NXC = CC::NXC, NAB = CC::NAB, SLOTN = CC::SLOTN;
+    constexpr int NP = 2 * LX + 1, NINTP = NP * NAB, SLOTP = NINTP | 1;
+    const SetId sid = decode_set(map, batch * 32 + lane, swapped);
+    double AB[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) AB[d] = prim.center[3 * sid.a + d] - prim.center[3 * sid.b + d];
+    const bool tr = swapped != 0;
+    for (int m = warp; m < NP; m += NW) {
+        double H0[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) H0[i] = 0.0;
+#pragma unroll 1
+        for (int c = 0; c < NXC; ++c) {
+            const double sc = __ldg(smat + m * NXC + c);          // warp-uniform
+            if (sc != 0.0) {
+                const double *src = TC + (size_t)lane * SLOTN + c * NAB;
+                static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(sc, src[decltype(ii)::value], H0[decltype(ii)::value]); });
+            }
+        }
+        hrr_store<LA, LB>(H0, AB, PR + (size_t)lane * SLOTP + m * NAB, tr);
+    }
+    __syncthreads();
+    batch_copy_out<NINTP, SLOTP>(PR, out, batch, map.nsets, warp * 32 + lane, NW * 32);
+    __syncthreads();
+}
+
 // ---- team plan: W warps, warp w owns the targets [w·NTW, (w+1)·NTW) (ordered by level) ------------------------------------
 template <int LX, int LA, int LB, int W>
 struct TeamCls {
@@ -393,13 +437,15 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
             double *__restrict__ out, int swapped, DfArgs df) {
     using CC = ChainCls<LX, LA, LB>;
     using TM = TeamCls<LX, LA, LB, W>;
-    constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NT = TM::NT, NTW = TM::NTW;
+    // MODE 3 (pure aux functions) needs the level-0 targets only
+    constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NT = MODE == 3 ? CC::NXC : TM::NT, NTW = (NT + W - 1) / W;
+    constexpr int NUBX = MODE == 3 ? cmax(TM::NUB, 32 * (((2 * LX + 1) * CC::NAB) | 1)) : TM::NUB;   // staging / pure region
     constexpr unsigned FULL = 0xffffffffu;
 
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]
     double *UB = TC + (size_t)32 * CC::SLOTN;                // [(ti − NXC)][i][set]
-    PartnerTab *pt = reinterpret_cast<PartnerTab *>(UB + TM::NUB + 4);
+    PartnerTab *pt = reinterpret_cast<PartnerTab *>(UB + NUBX + 4);
     if (threadIdx.x == 0) partner_tab_build<LX>(pt);
     __syncthreads();
 
@@ -472,7 +518,8 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
             }
         });
         __syncthreads();
-        chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+        if constexpr (MODE == 3) pure_epilogue<LX, LA, LB, W>(TC, UB, df.D, warp, lane, batch, map, prim, out, swapped);
+        else chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
     }
 }
 
@@ -481,7 +528,8 @@ cudaError_t team_launch(const SetMap &map, const DevShells &aux, const DevShells
                         const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                         cudaStream_t stream) {
     using TM = TeamCls<LX, LA, LB, W>;
-    constexpr size_t smem = TM::smem;
+    constexpr int NUBX = MODE == 3 ? cmax(TM::NUB, 32 * (((2 * LX + 1) * TM::CC::NAB) | 1)) : TM::NUB;
+    constexpr size_t smem = ((size_t)32 * TM::CC::SLOTN + NUBX + 4) * 8 + sizeof(PartnerTab);
     static_assert(smem <= 227 * 1024, "team kernel: batch does not fit in shared memory");
     // registers: accumulators + start vector + chain copy (doubles), two primitive records, Boys values, scalars
     constexpr int need = 2 * (TM::acc_doubles + 2 * TM::CC::NG) + 110;

@@ -23,7 +23,7 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
            "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family",
-           "lx_cart_to_pure", "lx_solid_matrix"]
+           "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes"]
 
 
 class lx_shells_t(C.Structure):
@@ -45,6 +45,10 @@ _lib.lx_schedule_num_integrals.argtypes = [C.c_void_p]
 _lib.lx_schedule_destroy.argtypes = [C.c_void_p]
 _lib.lx_cart_to_pure.argtypes = [C.c_int, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.lx_solid_matrix.argtypes = [C.c_int, C.c_void_p]
+_lib.lx_eri3_pure_workspace_bytes.restype = C.c_size_t
+_lib.lx_eri3_pure_workspace_bytes.argtypes = [C.c_int] * 6
+_lib.lx_eri3_batch_pure.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(lx_shells_t), C.POINTER(lx_shells_t), C.c_void_p,
+                                    C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
 _lib.lx_launch_count.restype = C.c_int64
 _lib.lx_eri3_batch.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(lx_shells_t), C.POINTER(lx_shells_t),
                                C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -249,6 +253,25 @@ def lx_df_J(sched, aux, prim, d, J=None, workspace=None, stream=None):
     _check(_lib.lx_df_J(sched.handle, C.byref(aux.struct), C.byref(prim.struct), d.data_ptr(), J.data_ptr(),
                         J.stride(0), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
     return J
+
+
+def lx_eri3_batch_pure(lx, la, lb, aux, prim, x_idx, pair_idx, out=None, workspace=None, stream=None, kmax=None):
+    """(X_m|ab) with solid-harmonic aux functions → out[npair, nx, 2lx+1, nc(la), nc(lb)] (device)."""
+    dev = aux.device
+    x_idx = _dev_i32(x_idx, dev)
+    pair_idx = _dev_i32(pair_idx, dev).reshape(-1, 2)
+    nx, npair = x_idx.numel(), pair_idx.shape[0]
+    if kmax is None:
+        kmax = kmax_pair(prim.host, pair_idx.cpu().numpy())
+    if out is None:
+        out = torch.empty((npair, nx, 2 * lx + 1, ncart(la), ncart(lb)), dtype=torch.float64, device=dev)
+    need = int(_lib.lx_eri3_pure_workspace_bytes(lx, la, lb, nx, npair, kmax))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+    _check(_lib.lx_eri3_batch_pure(lx, la, lb, C.byref(aux.struct), C.byref(prim.struct), x_idx.data_ptr(), nx,
+                                   pair_idx.data_ptr(), npair, kmax, out.data_ptr(), workspace.data_ptr(),
+                                   C.c_size_t(workspace.numel()), _stream_ptr(stream)))
+    return out
 
 
 def lx_cart_to_pure(lx, cart, out=None, stream=None):

@@ -258,3 +258,20 @@ def test_cart_to_pure_transform(lx, oracle, cls):
     _check(got.cpu().numpy(), ref)
     with pytest.raises(lx.LxError):                                   # in == out is refused
         lx._check(lx._lib.lx_cart_to_pure(lxa, 1, 1, cart.data_ptr(), cart.data_ptr(), None))
+
+
+@pytest.mark.parametrize("cls", [(2, 1, 1), (4, 2, 0), (3, 1, 2), (4, 1, 1), (2, 0, 0), (4, 2, 2), (1, 1, 0), (6, 1, 0), (5, 3, 1)])
+def test_eri3_batch_pure(lx, oracle, cls):
+    """Solid-harmonic aux functions: the fused path (team classes with lx >= 2: level-0 chain
+    targets of eq. 2 + projection in the epilogue) and the fallback (Cartesian + lx_cart_to_pure), mirrored classes
+    included, against oracle Cartesian integrals x the oracle's solid-harmonic matrix."""
+    import torch
+    from oracle import solid
+    lxa, la, lb = cls
+    cfg = gen.config2(lxa, la, lb, npair=37, nx=19) if lxa <= 4 and max(la, lb) <= 2 else gen.config3(lxa, la, lb, kprim=2, npair=9, nx=5)
+    aux, prim = lx.DeviceShells(cfg["aux"]), lx.DeviceShells(cfg["prim"])
+    got = lx.lx_eri3_batch_pure(lxa, la, lb, aux, prim, cfg["x_idx"], cfg["pair_idx"])
+    torch.cuda.synchronize()
+    ref = solid.cart_to_pure(lxa, oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"], cfg["pair_idx"]))
+    assert got.shape == ref.shape
+    _check(got.cpu().numpy(), ref)
