@@ -88,3 +88,33 @@ def test_chain_form_equals_oracle(oracle, E, LX):
                 worst = max(worst, abs(out[(c, a)] - ref[ic, ia]))
                 scale = max(scale, abs(ref[ic, ia]))
     assert worst <= 1e-13 * scale, (worst, scale)
+
+
+def test_closed_n_quantal_form_g5_g6():
+    """Reading G5/G6: the corrected closed form of the paper's eq. 8,
+        (B^t z)[a] = sum_{u <= min(a,t)} prod_i C(t_i,u_i) C(a_i,u_i) u_i!  w^(t-u) c^|u| z[a-u],
+    is the expansion of the chain operator B_i = w_i + c S_i, and its integer coefficients for a = t = (2,0,0) are the
+    1, 4, 2 of the worked example eq. 9 (the printed last coefficient 1 is a typo: tests/golden/cvrr2_example.txt)."""
+    import os
+    rng = np.random.default_rng(8)
+    E, LX = 4, 4
+    allA = [a for e in range(E + 1) for a in comps(e)]
+    z = {a: rng.normal() for a in allA}
+    w, cs = rng.normal(size=3), 0.37
+    for t in comps(LX) + comps(2) + comps(3):
+        # stepping: f <- w_i f[a] + c a_i f[a - 1_i]
+        f = dict(z)
+        for i in range(3):
+            for _ in range(t[i]):
+                f = {a: w[i] * f[a] + (cs * a[i] * f[tuple(a[d] - (d == i) for d in range(3))] if a[i] > 0 else 0.0) for a in allA}
+        for a in allA:
+            closed = 0.0
+            for u in itertools.product(*[range(min(a[i], t[i]) + 1) for i in range(3)]):
+                coef = 1
+                for i in range(3):
+                    coef *= math.comb(t[i], u[i]) * math.comb(a[i], u[i]) * math.factorial(u[i])
+                closed += coef * np.prod([w[i] ** (t[i] - u[i]) for i in range(3)]) * cs ** sum(u) * z[tuple(a[i] - u[i] for i in range(3))]
+            assert abs(closed - f[a]) <= 1e-12 * max(1.0, abs(f[a])), (t, a)
+    gold = [tuple(int(v) for v in ln.split()) for ln in open(os.path.join(os.path.dirname(__file__), "golden", "cvrr2_example.txt"))
+            if ln.strip() and not ln.startswith("#")]
+    assert gold == [(u, math.comb(2, u) ** 2 * math.factorial(u)) for u in range(3)] == [(0, 1), (1, 4), (2, 2)]
