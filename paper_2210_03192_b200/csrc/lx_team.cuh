@@ -397,14 +397,16 @@ __device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, dou
         double H0[NACC];
 #pragma unroll
         for (int i = 0; i < NACC; ++i) H0[i] = 0.0;
-#pragma unroll 1
-        for (int c = 0; c < NXC; ++c) {
-            const double sc = __ldg(smat + m * NXC + c);          // warp-uniform
-            if (sc != 0.0) {
-                const double *src = TC + (size_t)lane * SLOTN + c * NAB;
-                static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(sc, src[decltype(ii)::value], H0[decltype(ii)::value]); });
-            }
-        }
+        // unrolled over c: the loads of different c are independent (a rolled loop is bound by their latency); about three
+        // quarters of S_l[m][·] are zeros and skipped by a warp-uniform branch
+        const double *srow = smat + m * NXC;
+        const double *src0 = TC + (size_t)lane * SLOTN;
+        static_for<0, NXC>([&](auto ic) {
+            constexpr int c = decltype(ic)::value;
+            const double sc = __ldg(srow + c);                    // warp-uniform
+            if (sc != 0.0)
+                static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(sc, src0[c * NAB + decltype(ii)::value], H0[decltype(ii)::value]); });
+        });
         hrr_store<LA, LB>(H0, AB, PR + (size_t)lane * SLOTP + m * NAB, tr);
     }
     __syncthreads();
