@@ -340,36 +340,51 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
     }
     // a8 (DEFER: the caller copies the batch out later, overlapped with the start of the next batch)
     if constexpr (MODE == 0 && !DEFER) batch_copy_out<NINT, SLOTN>(TC, out, batch, map.nsets, warp * 32 + lane, NW * 32);
-    for (int s = warp; MODE != 0 && s < 32; s += NW) {
-        const long long sid_s = batch * 32 + s;
-        if (sid_s >= map.nsets) break;                    // warp-uniform
-        const double *FIN = TC + (size_t)s * SLOTN;       // finished shell-set, layout [c][a][b]
-        {
-            const int as = __shfl_sync(FULL, sid.a, s), bs = __shfl_sync(FULL, sid.b, s), xs_ = __shfl_sync(FULL, sid.x, s);
-            if constexpr (MODE == 1) {
-                // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
-                const double *Dab = df.D + (size_t)prim.bf_off[as] * df.ld + prim.bf_off[bs];
-                const double f = (as != bs) ? 2.0 : 1.0;
-                for (int c = lane; c < NXC; c += 32) {
-                    const double *Fc = FIN + c * NAB;
-                    double sum = 0.0;
-                    for (int ia = 0; ia < NA; ++ia)
+    // a9 / a10: LANE = shell-set here too, so all 32 sets of the batch are digested at once
+    if constexpr (MODE == 1) {
+        // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]: a lane sums its own set (the lanes of a batch mostly share the
+        // pair, so the D block is a broadcast load) and adds into its own γ entries; the warps split c
+        if (sid.live) {
+            const double *Dab = df.D + (size_t)prim.bf_off[sid.a] * df.ld + prim.bf_off[sid.b];
+            const double f = (sid.a != sid.b) ? 2.0 : 1.0;
+            double *gx = df.out + aux.bf_off[sid.x];
+            const double *FINl = TC + (size_t)lane * SLOTN;
+            for (int c = warp; c < NXC; c += NW) {
+                const double *Fc = FINl + c * NAB;
+                double sum = 0.0;
+                for (int ia = 0; ia < NA; ++ia)
 #pragma unroll
-                        for (int ib = 0; ib < NB; ++ib) sum = fma(Fc[ia * NB + ib], __ldg(Dab + (size_t)ia * df.ld + ib), sum);
-                    atomicAdd(df.out + aux.bf_off[xs_] + c, f * sum);
-                }
-            } else {
-                // J[bf(a)+ia, bf(b)+ib] += Σ_c (c|ab) d[bf(X)+c], mirrored
-                const double *dx = df.D + aux.bf_off[xs_];
-                const size_t ra0 = prim.bf_off[as], rb0 = prim.bf_off[bs];
-                for (int r = lane; r < NAB; r += 32) {
-                    double sum = 0.0;
+                    for (int ib = 0; ib < NB; ++ib) sum = fma(Fc[ia * NB + ib], __ldg(Dab + (size_t)ia * df.ld + ib), sum);
+                atomicAdd(gx + c, f * sum);
+            }
+        }
+    } else if constexpr (MODE == 2) {
+        // J[bf(a)+ia, bf(b)+ib] += Σ_X Σ_c (c|ab) d[bf(X)+c], mirrored: a lane contracts its own set with its d block, the
+        // lanes that share a shell pair (contiguous runs of the batch) are summed by shuffles, one atomic per run and element
+        const double *dx = df.D + aux.bf_off[sid.x];
+        const double *FINl = TC + (size_t)lane * SLOTN;
+        const unsigned livemask = __ballot_sync(FULL, sid.live);
+        for (int r = warp; r < NAB; r += NW) {
+            double v = 0.0;
+            if (sid.live) {
 #pragma unroll
-                    for (int c = 0; c < NXC; ++c) sum = fma(FIN[c * NAB + r], __ldg(dx + c), sum);
-                    const int ia = r / NB, ib = r - ia * NB;
+                for (int c = 0; c < NXC; ++c) v = fma(FINl[c * NAB + r], __ldg(dx + c), v);
+            }
+            const int ia = r / NB, ib = r - ia * NB;
+            unsigned rest = livemask;
+            while (rest) {                                    // warp-uniform loop over the runs of equal pairs
+                const int leader = __ffs(rest) - 1;
+                const int pl = __shfl_sync(FULL, sid.p, leader);
+                const unsigned grp = __ballot_sync(FULL, sid.live && sid.p == pl) & rest;
+                double sum = (grp >> lane) & 1u ? v : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+                if (lane == leader) {
+                    const size_t ra0 = prim.bf_off[sid.a], rb0 = prim.bf_off[sid.b];
                     atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
-                    if (as != bs) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
+                    if (sid.a != sid.b) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
                 }
+                rest &= ~grp;
             }
         }
     }
