@@ -150,7 +150,7 @@ int lx_cart_to_pure(int lx, int64_t nsets, int nab, const double *in, double *ou
 /* (X_m|ab) for SOLID-HARMONIC auxiliary functions (the paper's own target (ab|c); SURVEY.md §8(f)
  * NEXT-1): same arguments as lx_eri3_batch plus kmax_pair (largest K_a*K_b of the listed pairs), and
  *     out[npair][nx][2lx+1][nc(la)][nc(lb)],  m = -lx..lx.
- * Classes served by the team kernel with lx >= 2 run fused: for a pure ket eq. 2 is exact after
+ * Classes served by the team and chain kernels with lx >= 2 run fused: for a pure ket eq. 2 is exact after
  * projection, so only the level-0 chain targets are evaluated and the solid-harmonic matrix is applied in the epilogue.
  * Other classes evaluate the Cartesian shell-sets into the workspace and apply lx_cart_to_pure.  The workspace must hold
  * lx_eri3_pure_workspace_bytes(...) bytes (LX_ENOMEM otherwise); everything else as for lx_eri3_batch. */

@@ -17,7 +17,13 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
              double *__restrict__ out, int swapped, DfArgs df) {
     using CC = ChainCls<LX, LA, LB>;
     constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NXC = CC::NXC, NA = CC::NA, NB = CC::NB, NAB = CC::NAB;
-    constexpr int SLOTN = CC::SLOTN;
+    // MODE 3 (solid-harmonic aux functions, lx_team.cuh "MODE 3"): only the passes of the level-0 targets run, the (e0|c)
+    // slots are packed (NACC per ket component: the HRR writes to the pure region, which aliases the ring), one VRR1 level
+    constexpr bool PURE = MODE == 3;
+    constexpr int CSTR = PURE ? NACC : NAB;
+    constexpr int SLOTN = PURE ? ((NXC * NACC) | 1) : CC::SLOTN;
+    constexpr int ZBD = PURE ? cmax(CC::ZBD, 32 * (((2 * LX + 1) * NAB) | 1)) : CC::ZBD;
+    constexpr int NPE = PURE ? (NXC + CC::P.t1[0] - 1) / CC::P.t1[0] : CC::P.npass;   // passes that hold level-0 targets
     constexpr ChainTargets T = CC::T;
     constexpr ChainPlan P = CC::P;
     constexpr unsigned FULL = 0xffffffffu;
@@ -25,7 +31,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]: (e0|c), then the finished shell-set
     double *ZB = TC + (size_t)32 * SLOTN;                    // ring of start-vector buffers
-    double *hd0 = ZB + (size_t)CC::ZBD;                     // two header buffers: [9][32] doubles A, C, AB; po; 6 ints; kmax
+    double *hd0 = ZB + (size_t)ZBD;                     // two header buffers: [9][32] doubles A, C, AB; po; 6 ints; kmax
     PartnerTab *pt = reinterpret_cast<PartnerTab *>(hd0 + CC::HDRD + 4);
     if (threadIdx.x == 0) partner_tab_build<LX>(pt);
 
@@ -99,7 +105,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         // (warp w holds target T0 + w of the current pass, or idles through the barriers), warps [NCX, NCX + NPX) produce.
         constexpr int NCX = P.ncx, NPX = P.npx, NBUF = NPX + 1, ZREC = P.zrec;
         constexpr int BCOUNT = (NCX + 1) * 32;               // threads on a full[] / empty[] barrier
-        const int gtot = P.npass * kmax;                     // ring slots of the batch
+        const int gtot = NPE * kmax;                         // ring slots of the batch
         if (warp >= NCX) {
             // ================= producers: ring slots g = j, j + NPX, ... ======================================================
             const int j = warp - NCX;
@@ -107,9 +113,9 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             const double Cx = hd[3 * 32 + lane], Cy = hd[4 * 32 + lane], Cz = hd[5 * 32 + lane];
             const long long po = hpo[lane];
             const int xo0 = hi[0 * 32 + lane], Kab = hi[1 * 32 + lane], K = hi[2 * 32 + lane];
-            static_for<0, P.npass>([&](auto ipass) {
+            static_for<0, NPE>([&](auto ipass) {
                 constexpr int ip = decltype(ipass)::value;
-                constexpr int PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
+                constexpr int PLO = PURE ? 0 : P.plo[ip], NLV = PURE ? 1 : P.phi[ip] - P.plo[ip] + 1;
                 const int g0 = ip * kmax;
                 for (int q = ((j - g0) % NPX + NPX) % NPX; q < kmax; q += NPX) {
                     const int g = g0 + q, bsel = g % NBUF;
@@ -214,10 +220,11 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         } else {
             // ================= consumers ===========================================================================================
             double acc[NACC];                                // lives in the consumer branch only: producers keep their registers
-            static_for<0, P.npass>([&](auto ipass) {
+            static_for<0, NPE>([&](auto ipass) {
                 constexpr int ip = decltype(ipass)::value;
-                constexpr int T0 = P.t0[ip], NC = P.t1[ip] - P.t0[ip], PLO = P.plo[ip], NLV = P.phi[ip] - P.plo[ip] + 1;
-                static_assert(T0 + NC <= NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
+                constexpr int T0 = P.t0[ip], NC = (PURE ? cmin(P.t1[ip], NXC) : P.t1[ip]) - P.t0[ip];
+                constexpr int PLO = PURE ? 0 : P.plo[ip], NLV = PURE ? 1 : P.phi[ip] - P.plo[ip] + 1;
+                static_assert(PURE || T0 + NC <= NXC || ip == P.npass - 1, "levels p >= 1 must sit in the last pass");
 #pragma unroll
                 for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
                 const int g0 = ip * kmax;
@@ -237,18 +244,19 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
                     if (g + NBUF < gtot) named_arrive(1 + NBUF + bsel, BCOUNT);   // empty[bsel]
                 }
                 // level-0 targets go straight to their private Cartesian slot of TC
-                if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB>(T0 + warp, acc, TC, ZB, lane);
+                if (warp < NC && T0 + warp < NXC) target_drop<LX, LA, LB, CSTR, SLOTN>(T0 + warp, acc, TC, ZB, lane);
                 if constexpr (LX_CHAIN_REALIGN && CC::P.npass > 2 && ip + 1 < CC::P.npass) named_sync(15, NW * 32);
             });
             named_sync(15, NW * 32);                         // all ring traffic of the batch is done
             // the targets of the levels p >= 1 (all in the last pass) go to the staging area, which aliases the idle ring
-            if constexpr (CC::T.n > NXC) {
+            if constexpr (!PURE && CC::T.n > NXC) {
                 constexpr int T0L = P.t0[P.npass - 1], NCL = P.t1[P.npass - 1] - T0L;
                 if (warp < NCL && T0L + warp >= NXC) target_drop<LX, LA, LB>(T0L + warp, acc, TC, ZB, lane);
             }
         }
         __syncthreads();
-        chain_epilogue<LX, LA, LB, MODE, NW, true>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+        if constexpr (PURE) pure_epilogue<LX, LA, LB, NW, CSTR, SLOTN>(TC, ZB, df.D, warp, lane, batch, map, prim, out, swapped);
+        else chain_epilogue<LX, LA, LB, MODE, NW, true>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
     }
     // the last batch of this block (the epilogue ended with a block barrier)
     if constexpr (MODE == 0) {
@@ -265,7 +273,11 @@ cudaError_t chain_launch(const SetMap &map, const DevShells &aux, const DevShell
                          cudaStream_t stream) {
     using CC = ChainCls<LX, LA, LB>;
     constexpr int NW = CC::NW;
-    constexpr size_t smem = CC::smem;
+    // MODE 3: packed (e0|c) slots, the pure region aliases the ring (see the kernel)
+    constexpr int SLOT3 = (CC::NXC * CC::NACC) | 1, ZBD3 = cmax(CC::ZBD, 32 * (((2 * LX + 1) * CC::NAB) | 1));
+    constexpr size_t smem = MODE == 3 ? ((size_t)32 * SLOT3 + (size_t)ZBD3 + CC::HDRD + 4) * 8 + 2048 : CC::smem;
+    if constexpr (smem > 227 * 1024) return cudaErrorNotSupported;   // MODE 3 only: the caller falls back
+    else {
     // resident blocks per SM: shared memory, and registers (a consumer keeps NG + NACC doubles live)
     constexpr int by_smem = (int)((227 * 1024) / (smem + 1024));
     constexpr int regs = CC::E <= 2 ? 80 : (CC::E == 3 ? 128 : 168);
@@ -284,6 +296,7 @@ cudaError_t chain_launch(const SetMap &map, const DevShells &aux, const DevShell
     if (blocks > cap) blocks = cap;
     kern<<<(unsigned)blocks, NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
     return cudaGetLastError();
+    }
 }
 
 }  // namespace lx

@@ -46,6 +46,8 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         // fused solid-harmonic aux functions: team kernel only; the caller falls back to Cartesian + lx_cart_to_pure
         if constexpr (has_team && LX >= 2)
             return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+        else if constexpr (has_chain && LX >= 2)
+            return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
         else
             return cudaErrorNotSupported;
     } else {

@@ -222,12 +222,13 @@ __device__ __forceinline__ void partner_tab_build(PartnerTab *pt) {
 // Drop the contracted target ti (run-time, warp-uniform) of this lane's set: level 0 goes straight to its Cartesian slot
 // of TC, higher levels to the staging area UB[(ti − NXC)][i][lane]; both scaled back by a! (lx_chain.cuh header).
 // One copy of this code serves every target: code that runs once per batch must stay small (instruction cache).
-template <int LX, int LA, int LB>
+template <int LX, int LA, int LB, int CSTR = ChainCls<LX, LA, LB>::NAB, int SLOT = ChainCls<LX, LA, LB>::SLOTN>
 __device__ __forceinline__ void target_drop(int ti, const double *__restrict__ acc, double *__restrict__ TC,
                                             double *__restrict__ UB, int lane) {
     using CC = ChainCls<LX, LA, LB>;
     constexpr int NACC = CC::NACC, NXC = CC::NXC;
-    double *dst = ti < NXC ? TC + (size_t)lane * CC::SLOTN + ti * CC::NAB : UB + (size_t)(ti - NXC) * NACC * 32 + lane;
+    // TC slot of a set: SLOT doubles, CSTR per ket component (the defaults leave room for the in-place HRR)
+    double *dst = ti < NXC ? TC + (size_t)lane * SLOT + ti * CSTR : UB + (size_t)(ti - NXC) * NACC * 32 + lane;
     const int stride = ti < NXC ? 1 : 32;
     static_for<0, NACC>([&](auto ii) {
         constexpr int i = decltype(ii)::value;
@@ -396,12 +397,12 @@ __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const do
 // two-term relation eq. 2 is exact after projection: only the level-0 targets G_c = (Π B^c Z^{(Lx)}) are
 // evaluated, and (X_m|e0) = Σ_c S_l[m][c] G_c with the real solid harmonics S_lm (lx.h, lx_cart_to_pure).  Per (set = lane,
 // m): transform, HRR in registers, store into the pure region PR [set][m][a][b]; then the batch leaves coalesced.
-template <int LX, int LA, int LB, int NW>
+template <int LX, int LA, int LB, int NW, int CSTR = ChainCls<LX, LA, LB>::NAB, int SLOT = ChainCls<LX, LA, LB>::SLOTN>
 __device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, double *__restrict__ PR,
                                               const double *__restrict__ smat, int warp, int lane, long long batch,
                                               const SetMap &map, const DevShells &prim, double *__restrict__ out, int swapped) {
     using CC = ChainCls<LX, LA, LB>;
-    constexpr int NACC = CC::NACC, NXC = CC::NXC, NAB = CC::NAB, SLOTN = CC::SLOTN;
+    constexpr int NACC = CC::NACC, NXC = CC::NXC, NAB = CC::NAB;
     constexpr int NP = 2 * LX + 1, NINTP = NP * NAB, SLOTP = NINTP | 1;
     const SetId sid = decode_set(map, batch * 32 + lane, swapped);
     double AB[3];
@@ -415,12 +416,12 @@ __device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, dou
         // unrolled over c: the loads of different c are independent (a rolled loop is bound by their latency); about three
         // quarters of S_l[m][·] are zeros and skipped by a warp-uniform branch
         const double *srow = smat + m * NXC;
-        const double *src0 = TC + (size_t)lane * SLOTN;
+        const double *src0 = TC + (size_t)lane * SLOT;
         static_for<0, NXC>([&](auto ic) {
             constexpr int c = decltype(ic)::value;
             const double sc = __ldg(srow + c);                    // warp-uniform
             if (sc != 0.0)
-                static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(sc, src0[c * NAB + decltype(ii)::value], H0[decltype(ii)::value]); });
+                static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(sc, src0[c * CSTR + decltype(ii)::value], H0[decltype(ii)::value]); });
         });
         hrr_store<LA, LB>(H0, AB, PR + (size_t)lane * SLOTP + m * NAB, tr);
     }

@@ -260,7 +260,8 @@ def test_cart_to_pure_transform(lx, oracle, cls):
         lx._check(lx._lib.lx_cart_to_pure(lxa, 1, 1, cart.data_ptr(), cart.data_ptr(), None))
 
 
-@pytest.mark.parametrize("cls", [(2, 1, 1), (4, 2, 0), (3, 1, 2), (4, 1, 1), (2, 0, 0), (4, 2, 2), (1, 1, 0), (6, 1, 0), (5, 3, 1)])
+@pytest.mark.parametrize("cls", [(2, 1, 1), (4, 2, 0), (3, 1, 2), (4, 1, 1), (2, 0, 0), (4, 2, 2), (4, 1, 2), (3, 2, 2), (2, 2, 2),
+                                 (1, 1, 0), (6, 1, 0), (5, 3, 1)])
 def test_eri3_batch_pure(lx, oracle, cls):
     """Solid-harmonic aux functions: the fused path (team classes with lx >= 2: level-0 chain
     targets of eq. 2 + projection in the epilogue) and the fallback (Cartesian + lx_cart_to_pure), mirrored classes
