@@ -355,6 +355,34 @@ def main():
                   "screening": "none (all shell-sets computed)", "shell_sets": sched.num_sets, "integrals": sched.num_integrals,
                   "gamma_ms": ms["gamma"], "J_ms": ms["J"], "df_j_ms": ms["gamma"] + ms["J"],
                   "integrals_per_s": 2 * sched.num_integrals / ((ms["gamma"] + ms["J"]) * 1e-3)}
+        # ---- side measurement: the same sweep with SOLID-HARMONIC aux functions through
+        # lx_eri3_batch_pure (fused for Lx >= 2, Cartesian + transform for Lx <= 1); serial on one stream; not part of `value`
+        pure = None
+        if world == 1 and not args.no_df and not args.classes:
+            wsp = torch.empty(max(int(lx._lib.lx_eri3_pure_workspace_bytes(c[0], c[1], c[2], args.nx, args.npair, 9)) for c in classes),
+                              dtype=torch.uint8, device=dev)
+            n_pure = sum((2 * c[0] + 1) * ncart(c[1]) * ncart(c[2]) for c in classes) * nsets
+
+            def pure_step():
+                for i, c in enumerate(classes):
+                    da, dp, dx, dpr = devs[c]
+                    n = (2 * c[0] + 1) * ncart(c[1]) * ncart(c[2]) * nsets
+                    lx.lx_eri3_batch_pure(c[0], c[1], c[2], da, dp, dx, dpr, out=outs[i][:n], workspace=wsp, kmax=9)
+            pure_step()
+            torch.cuda.synchronize()
+            best = 1e30
+            for _ in range(3):
+                flush.fill_(1)
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                a0.record()
+                pure_step()
+                a1.record()
+                torch.cuda.synchronize()
+                best = min(best, a0.elapsed_time(a1))
+            pure = {"workload": "configs[1] with solid-harmonic aux functions (2Lx+1 components), one stream",
+                    "ms_per_step": best, "integrals_per_step": n_pure, "integrals_per_s": n_pure / (best * 1e-3),
+                    "shell_sets_per_s": nsets * len(classes) / (best * 1e-3)}
         per_class = {f"({c[0]}|{c[1]}{c[2]})": round(float(nint_set(c) * nsets / (m * 1e-3)), 1) for c, m in zip(classes, class_ms)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -367,7 +395,7 @@ def main():
                            "streams": f"{1 + len(side)} CUDA streams per step (independent classes overlap); the same classes launched "
                                       f"back to back on one stream take {serial_ms:.2f} ms (sum of per-class event times)"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-                "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df,
+                "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df, "pure_sweep": pure,
                 "integrals_per_s_per_class": per_class}
         print(json.dumps(line))
     if world > 1:
