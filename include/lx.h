@@ -58,8 +58,10 @@ typedef struct {
 } lx_shells_t;
 
 /* Library state.  lx_init builds the Boys-function interpolation table (PAPER.md:132 and eq. 19:
- * F_m(x) = ∫_0^1 y^{2m} exp(−x y²) dy) on the host in long double and uploads it to `device`; it also raises the
- * dynamic shared-memory limit of every kernel.  Idempotent.  lx_finalize frees the table. */
+ * F_m(x) = ∫_0^1 y^{2m} exp(−x y²) dy) on the host in long double and uploads it to `device`.  Idempotent for the same
+ * device; a call with another device moves the library there (the old tables are freed; one device at a time per
+ * process — the intended use is one process per GPU).  Kernel attributes (dynamic shared-memory limits) are set per
+ * device at the first launch of each kernel.  lx_finalize frees the tables. */
 int lx_init(int device);
 int lx_finalize(void);
 const char *lx_strerror(int status);
@@ -78,10 +80,23 @@ const char *lx_version(void);
  *   workspace: device scratch of at least lx_eri3_workspace_bytes(...) bytes (primitive-pair data, row a1).
  * nx == 0 or npair == 0 is a no-op returning LX_OK.
  * Errors: LX_EINVAL (null pointer with non-zero count, negative count), LX_EUNSUPPORTED, LX_ENOMEM, LX_ENOTINIT,
- * LX_ECUDA. */
+ * LX_ECUDA.
+ * Workspace contract: the record stride of the primitive-pair data is workspace_bytes / npair, so the workspace must be
+ * sized with kmax_pair >= max K_a*K_b over the listed pairs.  The lists live on the device, so the call itself cannot
+ * see a violation without synchronising: if a listed pair has more primitive pairs than the stride, nothing is read
+ * or written out of bounds, every integral of that pair comes back as NaN, and lx_async_status() reports LX_ENOMEM.
+ * With LX_CHECK=1 in the environment (read by lx_init; debug aid) the call first validates on the device, and
+ * synchronises: index range and class conformity of x_idx / pair_idx (LX_EINVAL) and the stride (LX_ENOMEM), and
+ * launches nothing if the check fails. */
 int lx_eri3_batch(int lx, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim,
                   const int32_t *x_idx, int nx, const int32_t *pair_idx, int npair, double *out,
                   void *workspace, size_t workspace_bytes, void *stream);
+
+/* Status of the asynchronous work issued since the last call of this function: LX_OK, LX_ENOMEM (a pair exceeded the
+ * workspace stride, see lx_eri3_batch) or LX_EINVAL (LX_CHECK=1 found an index out of range or a shell of the wrong
+ * class).  Reads one word from the device (synchronises with the legacy stream; the caller synchronises its own
+ * streams first) and clears it. */
+int lx_async_status(void);
 
 /* Workspace size for lx_eri3_batch: kmax_pair = max over listed pairs of K_a*K_b (contraction degrees). */
 size_t lx_eri3_workspace_bytes(int lx, int la, int lb, int nx, int npair, int kmax_pair);

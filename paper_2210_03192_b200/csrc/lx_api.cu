@@ -4,6 +4,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -28,8 +29,9 @@ struct State {
     // grow-only device arena for the host-buffer convenience path
     void *arena = nullptr;
     size_t arena_bytes = 0;
-    void *pinned = nullptr;
-    size_t pinned_bytes = 0;
+    // asynchronous status word in device memory, OR-ed into by the kernels (lx_async_status)
+    int *flag_dev = nullptr;
+    int check = 0;                   // LX_CHECK=1 in the environment (read by lx_init)
 };
 static State g;
 static std::mutex g_mu;
@@ -77,8 +79,10 @@ static void boys_table_host(std::vector<double> &tab) {
 // ------------------------------------------------------------------------------------------------ kernels
 // a1: primitive-pair data, one thread per (pair, primitive pair).  P by eq. 16, γ by eq. 14, K_ij = c_i c_j
 // exp(−ζaζb/γ |AB|²) (exponential factor of eq. 4).
+constexpr int FLAG_KSTRIDE = 1, FLAG_AUX_CLASS = 2, FLAG_PAIR_CLASS = 4, FLAG_RANGE = 8;
 __global__ void pair_data_kernel(DevShells prim, const int32_t *__restrict__ pair_list, int npair, int swapped,
-                                 const long long *__restrict__ pd_off, int kstride, int kiter, double *__restrict__ pd) {
+                                 const long long *__restrict__ pd_off, int kstride, int kiter, double *__restrict__ pd,
+                                 int *__restrict__ flag) {
     // flat index over pairs × kiter lanes; a lane walks ij = lane, lane+kiter, ... < K_a K_b
     const long long total = (long long)npair * kiter;
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
@@ -86,6 +90,9 @@ __global__ void pair_data_kernel(DevShells prim, const int32_t *__restrict__ pai
         const int lane = (int)(t - p * kiter);
         const int a = pair_list[2 * p + swapped], b = pair_list[2 * p + 1 - swapped];
         const int Ka = prim.K[a], Kb = prim.K[b];
+        // a pair with more primitive pairs than the record stride: the class kernels clamp the same way (no read past
+        // the record), the contraction is truncated and the status word says so (lx_async_status → LX_ENOMEM)
+        if (Ka * Kb > kstride && lane == 0) atomicOr(flag, FLAG_KSTRIDE);
         const int Kab = min(Ka * Kb, kstride);
         const double Ax = prim.center[3 * a], Ay = prim.center[3 * a + 1], Az = prim.center[3 * a + 2];
         const double Bx = prim.center[3 * b], By = prim.center[3 * b + 1], Bz = prim.center[3 * b + 2];
@@ -100,10 +107,33 @@ __global__ void pair_data_kernel(DevShells prim, const int32_t *__restrict__ pai
             pd[o + 1] = (za * Ax + zb * Bx) * ig;
             pd[o + 2] = (za * Ay + zb * By) * ig;
             pd[o + 3] = (za * Az + zb * Bz) * ig;
-            pd[o + 4] = ca * cb * exp(-za * zb * ig * r2);
+            // a truncated pair (see above) poisons its integrals: loud NaNs instead of a silently short contraction
+            pd[o + 4] = (Ka * Kb > kstride) ? __longlong_as_double(0x7ff8000000000000LL) : ca * cb * exp(-za * zb * ig * r2);
             pd[o + 5] = 0.5 * ig;
         }
     }
+}
+
+// LX_CHECK=1: class conformity of the index lists (the caller's contract otherwise, lx.h)
+__global__ void check_lists_kernel(DevShells aux, int naux, DevShells prim, int nprim, int lx_, int la, int lb,
+                                   const int32_t *__restrict__ x_idx, int nx, const int32_t *__restrict__ pair_idx, int npair,
+                                   int kstride, int *__restrict__ flag) {
+    int f = 0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < (long long)nx + npair; t += (long long)gridDim.x * blockDim.x) {
+        if (t < nx) {
+            const int x = x_idx[t];
+            if (x < 0 || x >= naux) f |= FLAG_RANGE;
+            else if (aux.L[x] != lx_) f |= FLAG_AUX_CLASS;
+        } else {
+            const int a = pair_idx[2 * (t - nx)], b = pair_idx[2 * (t - nx) + 1];
+            if (a < 0 || a >= nprim || b < 0 || b >= nprim) f |= FLAG_RANGE;
+            else {
+                if (prim.L[a] != la || prim.L[b] != lb) f |= FLAG_PAIR_CLASS;
+                if (prim.K[a] * prim.K[b] > kstride) f |= FLAG_KSTRIDE;
+            }
+        }
+    }
+    if (f) atomicOr(flag, f);
 }
 
 __global__ void boys_kernel(const double *__restrict__ tab, const double *__restrict__ T, int n, int mmax,
@@ -238,7 +268,7 @@ static int launch_pair_data(const DevShells &prim, const int32_t *pair_list, int
     const int threads = 256;
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 148LL * 16) blocks = 148LL * 16;
-    pair_data_kernel<<<(unsigned)blocks, threads, 0, st>>>(prim, pair_list, npair, swapped, pd_off, kstride, kiter, pd);
+    pair_data_kernel<<<(unsigned)blocks, threads, 0, st>>>(prim, pair_list, npair, swapped, pd_off, kstride, kiter, pd, g.flag_dev);
     g.launches++;
     LX_CUDA(cudaGetLastError());
     return LX_OK;
@@ -277,22 +307,45 @@ const char *lx_strerror(int status) {
     }
 }
 
+static void free_device_state() {
+    if (g.boys_tab) cudaFree(g.boys_tab);
+    if (g.arena) cudaFree(g.arena);
+    if (g.flag_dev) cudaFree(g.flag_dev);
+    for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
+        if (g.solid[l]) cudaFree(g.solid[l]);
+        g.solid[l] = nullptr;
+    }
+    g.boys_tab = nullptr;
+    g.arena = nullptr;
+    g.arena_bytes = 0;
+    g.flag_dev = nullptr;
+    g.ready = false;
+}
+
 int lx_init(int device) {
     std::lock_guard<std::mutex> lock(g_mu);
     if (g.ready && g.device == device) return LX_OK;
+    if (g.ready) {                       // moving to another device: the old tables are freed under the old device
+        cudaSetDevice(g.device);
+        free_device_state();
+    }
     LX_CUDA(cudaSetDevice(device));
+    {
+        const char *e = std::getenv("LX_CHECK");
+        g.check = (e && e[0] == '1') ? 1 : 0;
+    }
+    LX_CUDA(cudaMalloc((void **)&g.flag_dev, sizeof(int)));
+    LX_CUDA(cudaMemset(g.flag_dev, 0, sizeof(int)));
     cudaDeviceProp prop;
     LX_CUDA(cudaGetDeviceProperties(&prop, device));
     g.num_sms = prop.multiProcessorCount;
     std::vector<double> tab;
     boys_table_host(tab);
-    if (g.boys_tab) cudaFree(g.boys_tab);
     LX_CUDA(cudaMalloc(&g.boys_tab, tab.size() * sizeof(double)));
     LX_CUDA(cudaMemcpy(g.boys_tab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
     std::vector<std::vector<double>> mats;
     solid_matrices_host(mats);
     for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
-        if (g.solid[l]) cudaFree(g.solid[l]);
         LX_CUDA(cudaMalloc(&g.solid[l], mats[l].size() * sizeof(double)));
         LX_CUDA(cudaMemcpy(g.solid[l], mats[l].data(), mats[l].size() * sizeof(double), cudaMemcpyHostToDevice));
     }
@@ -303,19 +356,18 @@ int lx_init(int device) {
 
 int lx_finalize(void) {
     std::lock_guard<std::mutex> lock(g_mu);
-    if (g.boys_tab) cudaFree(g.boys_tab);
-    if (g.arena) cudaFree(g.arena);
-    if (g.pinned) cudaFreeHost(g.pinned);
-    for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
-        if (g.solid[l]) cudaFree(g.solid[l]);
-        g.solid[l] = nullptr;
-    }
-    g.boys_tab = nullptr;
-    g.arena = nullptr;
-    g.arena_bytes = 0;
-    g.pinned = nullptr;
-    g.pinned_bytes = 0;
-    g.ready = false;
+    if (g.ready) cudaSetDevice(g.device);
+    free_device_state();
+    return LX_OK;
+}
+
+int lx_async_status(void) {
+    if (!g.ready) return LX_ENOTINIT;
+    int f = 0;
+    LX_CUDA(cudaMemcpy(&f, g.flag_dev, sizeof(int), cudaMemcpyDeviceToHost));
+    if (f) LX_CUDA(cudaMemset(g.flag_dev, 0, sizeof(int)));
+    if (f & (FLAG_RANGE | FLAG_AUX_CLASS | FLAG_PAIR_CLASS)) return LX_EINVAL;
+    if (f & FLAG_KSTRIDE) return LX_ENOMEM;
     return LX_OK;
 }
 
@@ -418,8 +470,19 @@ int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shel
     const int cla = swapped ? lb : la, clb = swapped ? la : lb;
     DevShells dprim = dev_view(prim), daux = dev_view(aux);
     double *pd = reinterpret_cast<double *>(workspace);
-    // the stride must cover the largest K_a*K_b of the batch: checked on the host only through the documented
-    // contract lx_eri3_workspace_bytes(kmax_pair)
+    // The stride must cover the largest K_a*K_b of the batch (contract: lx_eri3_workspace_bytes(kmax_pair)).  The index
+    // lists live on the device, so a violation cannot be seen here without a synchronisation: the pre-pass records it in
+    // the status word (lx_async_status → LX_ENOMEM) and every kernel clamps to the stride, so nothing is read out of
+    // bounds.  LX_CHECK=1 validates stride and class conformity up front, synchronously.
+    if (g.check) {
+        if ((rc = lx_async_status()) != LX_OK) return rc;
+        check_lists_kernel<<<64, 256, 0, st>>>(daux, aux->nshell, dprim, prim->nshell, lx_, la, lb, x_idx, nx, pair_idx, npair,
+                                               kstride, g.flag_dev);
+        g.launches++;
+        LX_CUDA(cudaGetLastError());
+        LX_CUDA(cudaStreamSynchronize(st));
+        if ((rc = lx_async_status()) != LX_OK) return rc;
+    }
     if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kstride, pd, st)) != LX_OK) return rc;
     SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr};
     PairData pdat{pd, nullptr, kstride};

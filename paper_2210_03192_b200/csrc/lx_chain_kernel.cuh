@@ -63,7 +63,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         }
         const int a = map.pair_list[2 * p + swapped], b = map.pair_list[2 * p + 1 - swapped];
         const int x = map.x_list[xs];
-        const int Kab = prim.K[a] * prim.K[b];
+        const int Kab = min(prim.K[a] * prim.K[b], pdat.kstride);
         const int K = live ? Kab * aux.K[x] : 0;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -284,12 +284,8 @@ cudaError_t chain_launch(const SetMap &map, const DevShells &aux, const DevShell
     constexpr int by_regs = 65536 / (NW * 32 * regs);
     constexpr int BPS = cmax(1, cmin(cmin(by_smem, by_regs), 8));
     auto kern = chain_kernel<LX, LA, LB, MODE, NW, BPS>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
     if (map.nsets <= 0) return cudaSuccess;
     long long blocks = (map.nsets + 31) / 32;
     const long long cap = (long long)num_sms * BPS;

@@ -4,6 +4,7 @@
 // ζa, ζb; c = auxiliary (ket) shell X on centre C with exponent ζc; γ = ζa+ζb (eq. 14), ρ = γζc/(γ+ζc) (eq. 15),
 // P (eq. 16), AB = A−B (eq. 17), PC = P−C (eq. 18); [e 0|c]^(m) auxiliary integrals of §2.5.1 (lines 104–124).
 #pragma once
+#include <atomic>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -63,6 +64,21 @@ struct DfArgs {
     double *out;       // γ: gamma [naux_bf]                 J: J (nbf × nbf, ld)
     int ld;
 };
+
+// Function attributes are per device: raise the dynamic shared-memory limit of `kern` once per device of this process
+// (`mask` = one bit per device ordinal, a static of the launcher instantiation).
+template <class KernT>
+inline cudaError_t ensure_dyn_smem(KernT kern, size_t smem, std::atomic<unsigned long long> &mask) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (mask.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    mask.fetch_or(bit, std::memory_order_release);
+    return cudaSuccess;
+}
 
 // F_m(T)·scale for one m (thread-per-(set,m) evaluation).
 __device__ __forceinline__ double boys_one(const double *__restrict__ tab, int m, double T) {

@@ -191,7 +191,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             a = map.pair_list[2 * p + swapped];
             b = map.pair_list[2 * p + 1 - swapped];
             x = map.x_list[xs];
-            Kab = prim.K[a] * prim.K[b];
+            Kab = min(prim.K[a] * prim.K[b], pdat.kstride);   // never read past the pair's record (lx_api.cu: checked there)
             K = Kab * aux.K[x];
         }
         int kmax = K;
@@ -482,15 +482,11 @@ cudaError_t group_launch(const SetMap &map, const DevShells &aux, const DevShell
     constexpr BlockShape shape = pick_shape(G, (size_t)C::SLOT * 8);
     static_assert(shape.nthreads > 0, "class does not fit in shared memory");
     constexpr int NT = shape.nthreads;
-    static bool configured = false;
     // register cap: as many blocks per SM as shared memory allows, but never fewer than 96 registers per thread
     constexpr int MINB = cmax(1, cmin(shape.blocks_per_sm, 65536 / (NT * 96)));
     auto kern = group_kernel<LX, LA, LB, MODE, G, NT, MINB>;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shape.smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, shape.smem, configured); e != cudaSuccess) return e;
     if (map.nsets <= 0) return cudaSuccess;
     long long blocks = (map.nsets + shape.gpb - 1) / shape.gpb;
     const long long cap = (long long)num_sms * shape.blocks_per_sm;

@@ -238,7 +238,7 @@ lane_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
             a = map.pair_list[2 * p + swapped];
             b = map.pair_list[2 * p + 1 - swapped];
             x = map.x_list[xs];
-            Kab = prim.K[a] * prim.K[b];
+            Kab = min(prim.K[a] * prim.K[b], pdat.kstride);
             K = Kab * aux.K[x];
         }
         const int kmax = __reduce_max_sync(FULL, K);
@@ -525,12 +525,8 @@ cudaError_t lane_launch(const SetMap &map, const DevShells &aux, const DevShells
     constexpr int by_smem = (int)((227 * 1024) / (smem + 1024));
     constexpr int BPS = cmax(1, cmin(cmin(by_smem, 16), 65536 / (NWARPS * 32 * 128)));
     auto kern = lane_kernel<LX, LA, LB, MODE, NWARPS, BPS>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
     if (map.nsets <= 0) return cudaSuccess;
     const long long per_block = (long long)NWARPS * LC::SPW;
     long long blocks = (map.nsets + per_block - 1) / per_block;

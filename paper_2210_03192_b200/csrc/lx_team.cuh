@@ -472,7 +472,7 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
 
     for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
         const SetId sid = decode_set(map, batch * 32 + lane, swapped);
-        const int Kab = prim.K[sid.a] * prim.K[sid.b];
+        const int Kab = min(prim.K[sid.a] * prim.K[sid.b], pdat.kstride);
         const int K = sid.live ? Kab * aux.K[sid.x] : 0;
         const int kmax = __reduce_max_sync(FULL, K);
         const double A[3] = {prim.center[3 * sid.a], prim.center[3 * sid.a + 1], prim.center[3 * sid.a + 2]};
@@ -556,12 +556,8 @@ cudaError_t team_launch(const SetMap &map, const DevShells &aux, const DevShells
     constexpr int by_regs = 65536 / (W * 32 * regs);
     constexpr int BPS = cmax(1, cmin(cmin(by_smem, by_regs), 32));
     auto kern = team_kernel<LX, LA, LB, MODE, W, BPS>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
     if (map.nsets <= 0) return cudaSuccess;
     long long blocks = (map.nsets + 31) / 32;
     const long long cap = (long long)num_sms * BPS;

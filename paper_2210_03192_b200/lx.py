@@ -23,7 +23,7 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
            "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family",
-           "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes"]
+           "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status"]
 
 
 class lx_shells_t(C.Structure):
@@ -97,6 +97,11 @@ def lx_init(device=0):
 
 def lx_finalize():
     _check(_lib.lx_finalize())
+
+
+def lx_async_status():
+    """Status of the asynchronous work since the last call (LX_OK / LX_ENOMEM / LX_EINVAL); clears it."""
+    return int(_lib.lx_async_status())
 
 
 def lx_launch_count():
