@@ -30,11 +30,15 @@ METRIC = "3-center integrals/sec (class sweep, config 2)"
 UNIT = "integrals/s"
 WORKLOAD = "configs[1]: 45 classes (Lx 0..4 | La,Lb 0..2), K_total=9, 1024 pairs x 256 aux per class"
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk/SM x 2 x sm_max_mhz
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures under profiles/ (class -> bytes)
-NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): 1.071891e9 + 0.905e6}   # profiles/r01_ncu_chain_4_2_2.md
-# SURVEY.md §8(d) table, flops per shell-set at K = 9 for the classes it lists
+HBM_PEAK_GBS = 6555.5                                   # MEASURED_PEAKS.json (driver-written copy bandwidth), BASELINE.md §2
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the tracked ncu --set full summaries under
+# profiles/ (never measured by this run: ncu is not available inside a timed bench); class -> (bytes, source file)
+NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): (1.071891e9 + 0.905e6, "profiles/r01_ncu_chain_4_2_2.md")}
+# SURVEY.md §8(d) table, flops per shell-set for the classes it lists (K = 9 for config 2; config 3 as stated there)
 SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
                         (4, 1, 1): 29322, (4, 2, 2): 111054}
+SURVEY_FLOPS_CONFIG3 = {(6, 2, 2, 1): 43792, (5, 3, 3, 1): 70320, (6, 3, 3, 1): 116448, (4, 4, 4, 1): 93910,
+                        (5, 2, 2, 5): 566418}
 
 
 def ncart(l):
@@ -132,6 +136,167 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+def _time_calls(fn, reps, flush=None):
+    """CUDA-event times (ms) of `reps` calls of fn() on the current stream, each bracketed by a synchronize; the L2 is
+    flushed before every call when `flush` is given."""
+    import torch
+    out = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.fill_(1)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a0.record()
+        fn()
+        a1.record()
+        torch.cuda.synchronize()
+        out.append(a0.elapsed_time(a1))
+    return out
+
+
+def bench_config1(lx, dev):
+    """configs[0]: (d|pp), 64 pairs x 32 aux shells, K = 1 — launch-latency-sized: the time
+    of ONE lx_eri3_batch call (pre-pass + class kernel), median of 200 calls, and the back-to-back rate."""
+    import torch
+    cfg = gen.config1()
+    da, dp = lx.DeviceShells(cfg["aux"], dev), lx.DeviceShells(cfg["prim"], dev)
+    dx, dpr = torch.from_numpy(cfg["x_idx"]).to(dev), torch.from_numpy(cfg["pair_idx"]).to(dev)
+    out = torch.empty((64, 32, 6, 3, 3), dtype=torch.float64, device=dev)
+    ws = torch.empty(lx.lx_eri3_workspace_bytes(2, 1, 1, 32, 64, 1), dtype=torch.uint8, device=dev)
+
+    def call():
+        lx.lx_eri3_batch(2, 1, 1, da, dp, dx, dpr, out=out, workspace=ws, kmax=1)
+    for _ in range(10):
+        call()
+    ms = _time_calls(call, 200)
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a0.record()
+    for _ in range(200):
+        call()
+    a1.record()
+    torch.cuda.synchronize()
+    b2b = a0.elapsed_time(a1) / 200
+    nint = out.numel()
+    return {"workload": "configs[0]: class (2|11), 64 pairs x 32 aux shells, K=1, 110 592 integrals, 0.885 MB",
+            "us_per_call_median": 1e3 * float(np.median(ms)), "us_per_call_min": 1e3 * float(np.min(ms)),
+            "us_per_call_back_to_back": 1e3 * b2b, "integrals_per_s_back_to_back": nint / (b2b * 1e-3),
+            "launches_per_call": 2, "note": "device time between CUDA events around one C-ABI call; launch-latency-bound"}
+
+
+def bench_config3(lx, dev, costmodel):
+    """configs[2]: the five high-angular-momentum classes at 4096 pairs x 128 aux shells, one at a time (3.2-14.2 GB of
+    output each, far beyond the L2).  Per class: ms (median of 5 after 2 warm-ups), integrals/s, and the fraction of the
+    class's own floor max(8*nint / HBM peak, SURVEY.md §8(d) flops / FP64 peak)."""
+    import torch
+    res = {}
+    buf = None
+    for cls in gen.CONFIG3_CLASSES:
+        lxa, la, lb, k = cls
+        cfg = gen.config3(lxa, la, lb, kprim=k)
+        da, dp = lx.DeviceShells(cfg["aux"], dev), lx.DeviceShells(cfg["prim"], dev)
+        dx, dpr = torch.from_numpy(cfg["x_idx"]).to(dev), torch.from_numpy(cfg["pair_idx"]).to(dev)
+        nset = 4096 * 128
+        nint = nset * ncart(lxa) * ncart(la) * ncart(lb)
+        if buf is None or buf.numel() < nint:
+            buf = None
+            buf = torch.empty(nint, dtype=torch.float64, device=dev)
+        ws = torch.empty(lx.lx_eri3_workspace_bytes(lxa, la, lb, 128, 4096, k * k), dtype=torch.uint8, device=dev)
+
+        def call():
+            lx.lx_eri3_batch(lxa, la, lb, da, dp, dx, dpr, out=buf[:nint], workspace=ws, kmax=k * k)
+        call()
+        call()
+        ms = float(np.median(_time_calls(call, 5)))
+        t_hbm = 8.0 * nint / (HBM_PEAK_GBS * 1e9) * 1e3
+        fl_s, fl_m = SURVEY_FLOPS_CONFIG3[cls], costmodel.flops_per_set(lxa, la, lb, k * k)
+        t_f64 = fl_s * nset / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
+        floor = max(t_hbm, t_f64)
+        res[f"({lxa}|{la}{lb}) K={k * k}"] = {
+            "kernel": lx.lx_kernel_family(lxa, la, lb), "ms": ms, "integrals_per_s": nint / (ms * 1e-3),
+            "shell_sets_per_s": nset / (ms * 1e-3), "hbm_write_gbs": 8.0 * nint / (ms * 1e-3) / 1e9,
+            "floor_ms_hbm": t_hbm, "floor_ms_fp64_survey_flops": t_f64, "bound": "hbm" if t_hbm >= t_f64 else "alu",
+            "frac_of_floor": floor / ms, "tflops_survey_count": fl_s * nset / (ms * 1e-3) / 1e12,
+            "tflops_costmodel_count": fl_m * nset / (ms * 1e-3) / 1e12}
+    return {"workload": "configs[2]: 4096 pairs x 128 aux shells per class, 256 atoms >= 1.5 bohr apart in a 15-bohr cube",
+            "peaks": {"hbm_gbs": HBM_PEAK_GBS, "fp64_tflops": FP64_NOMINAL_TFLOPS}, "classes": res}
+
+
+def _df_model_flops(costmodel, aux, prim, pairs, qx, qp, tau):
+    """Cost-model flops of one DF pass: sum over (aux L,K) x (pair La,Lb,KaKb) buckets of surviving sets x flops/set."""
+    La, Lb = prim.L[pairs[:, 0]], prim.L[pairs[:, 1]]
+    la, lb = np.maximum(La, Lb), np.minimum(La, Lb)
+    kab = prim.K[pairs[:, 0]] * prim.K[pairs[:, 1]]
+    key = (la.astype(np.int64) * 8 + lb) * 4096 + kab
+    total = 0.0
+    for lxa in np.unique(aux.L):
+        for kx in np.unique(aux.K[aux.L == lxa]):
+            sel = (aux.L == lxa) & (aux.K == kx)
+            if qx is None:
+                cnt = np.full(len(pairs), int(sel.sum()), dtype=np.int64)
+            else:
+                qs = np.sort(qx[sel])
+                # survivors: qx >= tau / qp  (the schedule takes the decision as qx*qp >= tau; the model only needs counts)
+                with np.errstate(divide="ignore"):
+                    cnt = len(qs) - np.searchsorted(qs, tau / np.maximum(qp, 1e-300), side="left")
+            for kk in np.unique(key):
+                m = key == kk
+                n = int(cnt[m].sum())
+                if n:
+                    c = int(kk // 4096)
+                    total += n * costmodel.flops_per_set(int(lxa), c // 8, c % 8, int(kk % 4096) * int(kx))
+    return total
+
+
+def bench_df(lx, dev, costmodel, cfg, name, reps, unscreened=False):
+    """BASELINE.json metric "DF-J time": integral-direct gamma and J through lx_df_gamma / lx_df_J with Schwarz screening at
+    the config's tau.  The Schwarz factors are made on the GPU (lx_schwarz_*_host), the schedule on the host; both are
+    once-per-basis steps, timed and reported beside the per-iteration DF-J time, not inside it."""
+    import torch
+    aux, prim, pairs, tau = cfg["aux"], cfg["prim"], cfg["pair_idx"], cfg["tau"]
+    ha, hp = lx.HostShells(aux), lx.HostShells(prim)
+    t0 = time.perf_counter()
+    qx = lx.lx_schwarz_aux_host(ha)
+    qp = lx.lx_schwarz_pair_host(hp, pairs)
+    t_q = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    sched = lx.Schedule(ha, hp, qx, qp, pairs, tau)
+    t_s = time.perf_counter() - t0
+    da, dp = lx.DeviceShells(ha, dev), lx.DeviceShells(hp, dev)
+    D, d = torch.from_numpy(cfg["D"]).to(dev), torch.from_numpy(cfg["d"]).to(dev)
+    ws = torch.empty(sched.workspace_bytes, dtype=torch.uint8, device=dev)
+    gam = torch.empty(aux.nbf, dtype=torch.float64, device=dev)
+    J = torch.empty((prim.nbf, prim.nbf), dtype=torch.float64, device=dev)
+
+    def run(sc):
+        lx.lx_df_gamma(sc, da, dp, D, gamma=gam, workspace=ws)
+        torch.cuda.synchronize()
+        mg = min(_time_calls(lambda: lx.lx_df_gamma(sc, da, dp, D, gamma=gam, workspace=ws), reps))
+        lx.lx_df_J(sc, da, dp, d, J=J, workspace=ws)
+        torch.cuda.synchronize()
+        mj = min(_time_calls(lambda: lx.lx_df_J(sc, da, dp, d, J=J, workspace=ws), reps))
+        return mg, mj
+    mg, mj = run(sched)
+    lhs, rhs = float(gam @ d), float((J * D).sum())
+    fl = _df_model_flops(costmodel, aux, prim, pairs, qx, qp, tau)
+    floor_ms = fl / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
+    res = {"workload": name, "screening": f"Schwarz, tau = {tau:g}, factors made on the GPU (lx_schwarz_aux_host / lx_schwarz_pair_host)",
+           "nbf": prim.nbf, "naux": aux.nbf, "shell_pairs": len(pairs), "aux_shells": aux.nshell,
+           "shell_sets": sched.num_sets, "integrals": sched.num_integrals,
+           "surviving_fraction": sched.num_sets / (len(pairs) * aux.nshell),
+           "gamma_ms": mg, "J_ms": mj, "df_j_ms": mg + mj,
+           "integrals_per_s": 2 * sched.num_integrals / ((mg + mj) * 1e-3),
+           "fp64_floor_ms_per_pass_costmodel": floor_ms, "frac_of_fp64_floor": 2 * floor_ms / (mg + mj),
+           "check_gamma_dot_d": lhs, "check_J_dot_D": rhs, "check_rel_diff": abs(lhs - rhs) / max(abs(lhs), 1e-300),
+           "schwarz_s": t_q, "schedule_s": t_s}
+    if unscreened:
+        s0 = lx.Schedule(ha, hp, None, None, pairs, 0.0)
+        ug, uj = run(s0)
+        res["unscreened"] = {"shell_sets": s0.num_sets, "integrals": s0.num_integrals, "gamma_ms": ug, "J_ms": uj,
+                             "integrals_per_s": 2 * s0.num_integrals / ((ug + uj) * 1e-3)}
+    return res
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -144,11 +309,16 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--streams", type=int, default=2, help="CUDA streams the classes of a step are spread over")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-df", action="store_true", help="skip the DF-J (config 4) side measurement")
+    ap.add_argument("--no-df", action="store_true", help="skip the DF-J (configs 4, 5) and solid-harmonic side measurements")
+    ap.add_argument("--no-side", action="store_true", help="skip the config 1 / config 3 side measurements")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py --gpus {args.gpus} but WORLD_SIZE={world}: launch N ranks with "
+                         f"`python -m torch.distributed.run --nnodes=1 --nproc-per-node {args.gpus} --master-addr 127.0.0.1 "
+                         f"bench.py --gpus {args.gpus} ...` (one process per GPU)")
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
@@ -168,7 +338,7 @@ def main():
     classes = gen.CONFIG2_CLASSES
     if args.classes:
         classes = [tuple(int(v) for v in c.split(",")) for c in args.classes.split(";")]
-    seed = 2 + 1000 * rank
+    seed = 2 + 1000 * rank                    # config index; other ranks draw their own batch
     host, devs = {}, {}
     for c in classes:
         cfg = gen.config2(*c, npair=args.npair, nx=args.nx, seed=seed)
@@ -313,7 +483,9 @@ def main():
         achieved = fl_set * nsets / t_top / 1e12
         roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family(*canon)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
                     "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
-                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(canon), "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(canon, (None, None))[0],
+                    "traffic_source": NCU_DRAM_BYTES_PER_LAUNCH.get(canon, (None, "no ncu capture of this class under profiles/"))[1],
+                    "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
                     "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
                     "flops_per_set_survey": fl_survey,
                     "frac_with_survey_flops": (fl_survey * nsets / t_top / 1e12 / FP64_NOMINAL_TFLOPS) if fl_survey else None,
@@ -328,33 +500,15 @@ def main():
             n, t, cores = oracle_sample(classes, npair_s, nx_s, seed=2)
             cpu = {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
                    "sample": f"first {npair_s} pairs x {nx_s} aux shells of each of the 45 classes ({n} integrals, {t:.1f} s)"}
-        # ---- side measurement (BASELINE.json metric "DF-J time"): integral-direct gamma and J on configs[3] (64 atoms,
-        # 960 AO x 6 784 Cartesian DFAO) through lx_df_gamma / lx_df_J, all shell-sets (Schwarz factors are oracle data:
-        # the screened path is covered by the parity tests, not timed here); not part of `value`
-        df = None
+        # ---- side measurements: BASELINE.json metric "DF-J time" on configs[3] and configs[4] at their stated (Schwarz-
+        # screened) configuration, configs[2] per class and configs[0] per call; none of them is part of `value`
+        df = df5 = c1 = c3 = None
         if world == 1 and not args.no_df and not args.classes:
-            c4 = gen.config4()
-            h4a, h4p = lx.HostShells(c4["aux"]), lx.HostShells(c4["prim"])
-            sched = lx.Schedule(h4a, h4p, None, None, c4["pair_idx"], 0.0)
-            d4a, d4p = lx.DeviceShells(h4a, dev), lx.DeviceShells(h4p, dev)
-            D4, v4 = torch.from_numpy(c4["D"]).to(dev), torch.from_numpy(c4["d"]).to(dev)
-            ms = {}
-            for name, fn, arg in (("gamma", lx.lx_df_gamma, D4), ("J", lx.lx_df_J, v4)):
-                fn(sched, d4a, d4p, arg)
-                torch.cuda.synchronize()
-                best = 1e30
-                for _ in range(3):
-                    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a0.record()
-                    fn(sched, d4a, d4p, arg)
-                    a1.record()
-                    torch.cuda.synchronize()
-                    best = min(best, a0.elapsed_time(a1))
-                ms[name] = best
-            df = {"workload": "configs[3]: 64-atom cluster, nbf 960, naux 6784 (Cartesian), 73920 unique shell pairs x 1344 aux shells",
-                  "screening": "none (all shell-sets computed)", "shell_sets": sched.num_sets, "integrals": sched.num_integrals,
-                  "gamma_ms": ms["gamma"], "J_ms": ms["J"], "df_j_ms": ms["gamma"] + ms["J"],
-                  "integrals_per_s": 2 * sched.num_integrals / ((ms["gamma"] + ms["J"]) * 1e-3)}
+            df = bench_df(lx, dev, costmodel, gen.config4(), "configs[3]: 64-atom cluster, 960 AO x 6 784 Cartesian DFAO", 3, unscreened=True)
+            df5 = bench_df(lx, dev, costmodel, gen.config5(), "configs[4]: 256-atom cluster, 8 960 AO x 54 016 Cartesian DFAO, integral-direct", 1)
+        if world == 1 and not args.no_side and not args.classes:
+            c1 = bench_config1(lx, dev)
+            c3 = bench_config3(lx, dev, costmodel)
         # ---- side measurement: the same sweep with SOLID-HARMONIC aux functions through
         # lx_eri3_batch_pure (fused for Lx >= 2, Cartesian + transform for Lx <= 1); serial on one stream; not part of `value`
         pure = None
@@ -395,7 +549,8 @@ def main():
                            "streams": f"{1 + len(side)} CUDA streams per step (independent classes overlap); the same classes launched "
                                       f"back to back on one stream take {serial_ms:.2f} ms (sum of per-class event times)"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-                "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df, "pure_sweep": pure,
+                "shell_sets_per_s": value / ints_per_step * nsets * len(classes), "df_config4": df, "df_config5": df5,
+                "config1": c1, "config3": c3, "pure_sweep": pure,
                 "integrals_per_s_per_class": per_class}
         print(json.dumps(line))
     if world > 1:

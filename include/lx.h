@@ -101,6 +101,20 @@ int lx_async_status(void);
 /* Workspace size for lx_eri3_batch: kmax_pair = max over listed pairs of K_a*K_b (contraction degrees). */
 size_t lx_eri3_workspace_bytes(int lx, int la, int lb, int nx, int npair, int kmax_pair);
 
+/* Schwarz factors on the GPU (SURVEY.md §8(c) "Schwarz factors", §8(f) NEXT-2; "identical screening"):
+ *     q_aux[X]   = sqrt(max_c (X_c|X_c))        for every shell of `aux`            (2-centre Coulomb integrals)
+ *     q_pair[k]  = sqrt(max_{a,b} (a b|a b))    for every listed primary shell pair  (diagonal 4-centre integrals)
+ * so that |(X_c|a b)| <= q_aux[X] q_pair[k] for every component (Cauchy-Schwarz).  These are the arrays
+ * lx_schedule_create takes.  HOST in, HOST out: every array member of the table, pair_idx [npair*2] and the result
+ * are host pointers; the call uploads the table, evaluates the factors on the device (Hermite-Gaussian expansion of the
+ * pair densities, one thread per shell / shell pair, FP64) and returns after the result is complete.  Run once per
+ * basis; not part of the per-iteration path.  Accuracy: relative error <= 1e-12 against the long-double oracle
+ * (tests/test_gpu_schwarz.py), so a screening decision q_aux*q_pair < tau can differ from one taken with exact factors
+ * only for products within 1e-12 (relative) of tau.
+ * Errors: LX_EINVAL, LX_EUNSUPPORTED (L outside the compiled range), LX_ENOTINIT, LX_ECUDA. */
+int lx_schwarz_aux_host(const lx_shells_t *aux_host, double *q_aux_host);
+int lx_schwarz_pair_host(const lx_shells_t *prim_host, const int32_t *pair_idx_host, int npair, double *q_pair_host);
+
 /* Schedule — SURVEY.md §8(a) row a0; PAPER.md:54 (batches per class), :365 ("identical screening").
  * Built once per basis on the HOST from host copies of the shell tables.  Buckets aux shells by L and shell pairs
  * by (La, Lb) (pairs with La < Lb are stored swapped), orders every bucket by contraction degree and then by

@@ -13,6 +13,7 @@
 
 #include "lx_common.cuh"
 #include "lx_dispatch.h"
+#include "lx_state.h"
 #include "lx_team.cuh"
 
 namespace lx {
@@ -45,6 +46,12 @@ static int cuda_fail(cudaError_t e) {
         cudaError_t _e = (expr);                      \
         if (_e != cudaSuccess) return cuda_fail(_e);  \
     } while (0)
+
+bool state_ready() { return g.ready; }
+const double *state_boys_tab() { return g.boys_tab; }
+int state_num_sms() { return g.num_sms; }
+void state_count_launches(int n) { g.launches += n; }
+int state_cuda_fail(int e) { return cuda_fail((cudaError_t)e); }
 
 static const launch_fn k_launch[4][7] = {
     {launch_lx0_mode0, launch_lx1_mode0, launch_lx2_mode0, launch_lx3_mode0, launch_lx4_mode0, launch_lx5_mode0, launch_lx6_mode0},

@@ -80,6 +80,18 @@ inline cudaError_t ensure_dyn_smem(KernT kern, size_t smem, std::atomic<unsigned
     return cudaSuccess;
 }
 
+// Which shell of a pair carries the VRR (eq. 3 builds [e0|0] on centre A, eq. 1 then transfers onto b).  The transfer
+// (x−B)^b = Σ_k C(b,k) AB^{b−k} (x−A)^k cancels by (|AB|/σ)^{Lb} when the product Gaussian sits near B (ζb >> ζa): the
+// moments about A are then of size |AB|^e while the result is of size σ^e.  Building on the shell with the LARGER
+// (most diffuse) exponent keeps P near A and the transfer free of cancellation; for La = Lb the two roles can be
+// exchanged per shell pair at no cost (measured on config 3: 1e-12 -> 1e-14 of the batch maximum).
+__device__ __forceinline__ double shell_min_zeta(const DevShells &s, int i) {
+    const int o = s.prim_off[i], k = s.K[i];
+    double m = s.zeta[o];
+    for (int j = 1; j < k; ++j) m = fmin(m, s.zeta[o + j]);
+    return m;
+}
+
 // F_m(T)·scale for one m (thread-per-(set,m) evaluation).
 __device__ __forceinline__ double boys_one(const double *__restrict__ tab, int m, double T) {
     if (T < (double)BOYS_TMAX) {

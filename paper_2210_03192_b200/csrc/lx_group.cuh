@@ -174,6 +174,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         const long long sid = sbase + grp;
         const bool live = sid < map.nsets;
         int p = 0, x = 0, a = 0, b = 0, Kab = 1, K = 0;
+        bool tr = MODE == 0 && swapped != 0;                // caller's order is [c][b][a]: transposed store
         if (live) {
             int xs;
             if (map.cum == nullptr) {
@@ -193,6 +194,12 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
             x = map.x_list[xs];
             Kab = min(prim.K[a] * prim.K[b], pdat.kstride);   // never read past the pair's record (lx_api.cu: checked there)
             K = Kab * aux.K[x];
+            if constexpr (LA == LB && LB > 0) {              // the VRR runs on the shell with the larger exponents (lx_common.cuh)
+                if (shell_min_zeta(prim, b) > shell_min_zeta(prim, a)) {
+                    const int t = a; a = b; b = t;
+                    tr = !tr;
+                }
+            }
         }
         int kmax = K;
         if constexpr (G < 32) kmax = __reduce_max_sync(0xffffffffu, K);   // groups of one warp step together
@@ -406,7 +413,7 @@ group_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         if (K > 0) {
             if constexpr (MODE == 0) {
                 double *o = out + sid * C::NINT;
-                if (!swapped || LB == 0) {
+                if (!tr || LB == 0) {
                     for (int r = lane; r < C::NINT; r += G) o[r] = FIN[r];
                 } else {                                          // caller's order is [c][b][a]
                     for (int r = lane; r < C::NINT; r += G) {

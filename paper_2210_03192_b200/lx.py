@@ -23,7 +23,8 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
            "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family",
-           "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status"]
+           "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status",
+           "lx_schwarz_aux_host", "lx_schwarz_pair_host"]
 
 
 class lx_shells_t(C.Structure):
@@ -194,6 +195,25 @@ def lx_eri3_batch_host(lx, la, lb, aux_host, prim_host, x_idx, pair_idx, out=Non
     _check(_lib.lx_eri3_batch_host(lx, la, lb, C.byref(aux_host.struct), C.byref(prim_host.struct),
                                    x_idx.ctypes.data, nx, pair_idx.ctypes.data, npair, out.ctypes.data))
     return out
+
+
+_lib.lx_schwarz_aux_host.argtypes = [C.POINTER(lx_shells_t), C.c_void_p]
+_lib.lx_schwarz_pair_host.argtypes = [C.POINTER(lx_shells_t), C.c_void_p, C.c_int, C.c_void_p]
+
+
+def lx_schwarz_aux_host(aux_host):
+    """Q_X = sqrt(max_c (X_c|X_c)) per aux shell, evaluated on the GPU; HostShells in, numpy out."""
+    q = np.zeros(aux_host.nshell, dtype=np.float64)
+    _check(_lib.lx_schwarz_aux_host(C.byref(aux_host.struct), q.ctypes.data))
+    return q
+
+
+def lx_schwarz_pair_host(prim_host, pair_idx):
+    """Q_ab = sqrt(max_ab (ab|ab)) per listed primary shell pair, evaluated on the GPU; HostShells in, numpy out."""
+    pair_idx = np.ascontiguousarray(pair_idx, dtype=np.int32).reshape(-1, 2)
+    q = np.zeros(len(pair_idx), dtype=np.float64)
+    _check(_lib.lx_schwarz_pair_host(C.byref(prim_host.struct), pair_idx.ctypes.data, len(pair_idx), q.ctypes.data))
+    return q
 
 
 class Schedule:

@@ -49,3 +49,37 @@ def bruteforce_primitive(c, a, b, C, A, B, zc, za, zb, nt=48, nh=12.0, step=0.22
             prod *= h2 * hs * float(np.sum(f * g[:, None]))
         total += w * dudt * prod
     return 2.0 / np.sqrt(np.pi) * total
+
+
+def bruteforce_pair_diagonal(a, b, A, B, za, zb, nt=48, nh=12.0, step=0.22):
+    """(ab|ab) for ONE unnormalised primitive pair by the same plain quadrature as bruteforce_primitive (no Boys
+    function, no recurrence): both electrons carry the product (x-A)^a (x-B)^b exp(-za (x-A)^2 - zb (x-B)^2).
+        1/r12 = (2/sqrt(pi)) int_0^inf exp(-u^2 r12^2) du,  u = sqrt(rho) t / sqrt(1-t^2),  rho = p/2, p = za + zb."""
+    p = za + zb
+    rho = 0.5 * p
+    tn, tw = np.polynomial.legendre.leggauss(nt)
+    tn = 0.5 * (tn + 1.0)
+    tw = 0.5 * tw
+    total = 0.0
+    for t, w in zip(tn, tw):
+        u2 = rho * t * t / (1.0 - t * t)
+        dudt = np.sqrt(rho) * (1.0 - t * t) ** -1.5
+        prod = 1.0
+        for ax in range(3):
+            P = (za * A[ax] + zb * B[ax]) / p
+            deg = a[ax] + b[ax]
+            h2 = step / np.sqrt(p)
+            n2 = int(np.ceil(nh / step)) + 8 * (2 * deg + 1)
+            x2 = P + h2 * np.arange(-n2, n2 + 1)
+            al = u2 + p
+            hs = step / np.sqrt(al)
+            ns = int(np.ceil(nh / step)) + 8 * (deg + 1)
+            k = hs * np.arange(-ns, ns + 1)
+            s0 = -p * (x2 - P) / al
+            s = s0[:, None] + k[None, :]
+            x1 = x2[:, None] + s
+            f = ((x1 - A[ax]) ** a[ax]) * ((x1 - B[ax]) ** b[ax]) * np.exp(-za * (x1 - A[ax]) ** 2 - zb * (x1 - B[ax]) ** 2 - u2 * s * s)
+            g = ((x2 - A[ax]) ** a[ax]) * ((x2 - B[ax]) ** b[ax]) * np.exp(-za * (x2 - A[ax]) ** 2 - zb * (x2 - B[ax]) ** 2)
+            prod *= h2 * hs * float(np.sum(f * g[:, None]))
+        total += w * dudt * prod
+    return 2.0 / np.sqrt(np.pi) * total

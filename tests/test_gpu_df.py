@@ -140,6 +140,13 @@ def test_df_config5_sampled(lx, oracle):
         sum(int(np.sum(qp[i:i + 65536, None] * qx[None, :] >= tau)) for i in range(0, len(qp), 65536))
     sched, gamma, J = _gpu_df(lx, aux, prim, pairs, qx, qp, tau, c5["D"], c5["d"])
     assert sched.num_sets == nsets_ref                                       # identical screening decisions
+    # the GPU-made Schwarz factors (what bench.py uses) against the oracle's, all 3.3 M pairs
+    gx, gp = lx.lx_schwarz_aux_host(lx.HostShells(aux)), lx.lx_schwarz_pair_host(lx.HostShells(prim), pairs)
+    big = qp >= 1e-30
+    eq = max(float(np.max(np.abs(gx - qx) / qx)), float(np.max(np.abs(gp[big] - qp[big]) / qp[big])))
+    nsets_g = sum(int(np.sum(gp[i:i + 65536, None] * gx[None, :] >= tau)) for i in range(0, len(gp), 65536))
+    print(f"config 5: GPU Schwarz factors rel. error {eq:.2e}; surviving sets oracle {nsets_ref}, GPU factors {nsets_g}")
+    assert eq <= 1e-12 and abs(nsets_g - nsets_ref) <= 1e-9 * nsets_ref
     gsel = np.concatenate([np.arange(aux.bf_off[x], aux.bf_off[x + 1]) for x in x_sel])
     eg = _relerr(gamma[gsel], g_ref[gsel])
     mask = np.zeros((prim.nbf, prim.nbf), dtype=bool)

@@ -100,3 +100,18 @@ def test_df_selection_is_partial_sum(oracle):
     g2, J2, _, _ = oracle.df_gamma_J(aux, prim, pairs, qx, qp, 1e-12, D=D, d=d, p_sel=rest)
     assert np.linalg.norm(g1 + g2 - g_all) < 1e-14 * np.linalg.norm(g_all)
     assert np.linalg.norm(J1 + J2 - J_all) < 1e-14 * np.linalg.norm(J_all)
+
+
+def test_schwarz_pair_against_bruteforce_quadrature(oracle):
+    """Q_ab for La+Lb > 0 (only the one-sided Cauchy-Schwarz bound pinned it): (ab|ab) of one (p,s) and one
+    (d,p) primitive pair by plain quadrature (helpers.bruteforce_pair_diagonal: independent of Boys, of the Hermite
+    coefficients and of every recurrence); Q_ab^2 must equal the largest diagonal element."""
+    from helpers import bruteforce_pair_diagonal
+    comps = lambda l: [(x, y, l - x - y) for x in range(l, -1, -1) for y in range(l - x, -1, -1)]
+    for (la, lb, A, B, za, zb) in [(1, 0, np.array([0.2, -0.1, 0.3]), np.array([-0.4, 0.5, 0.1]), 0.9, 1.4),
+                                   (2, 1, np.array([0.0, 0.3, -0.2]), np.array([0.7, -0.4, 0.5]), 1.1, 0.6)]:
+        prim = table([(la, A, [za], [1.0]), (lb, B, [zb], [1.0])])
+        q = oracle.schwarz_pair(prim, [[0, 1]])[0]
+        diag = [bruteforce_pair_diagonal(ca, cb, A, B, za, zb) for ca in comps(la) for cb in comps(lb)]
+        assert min(diag) > 0
+        assert abs(q * q - max(diag)) <= 2e-11 * max(diag), (q * q, max(diag))
