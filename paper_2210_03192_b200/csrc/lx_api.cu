@@ -14,7 +14,7 @@
 #include "lx_common.cuh"
 #include "lx_dispatch.h"
 #include "lx_state.h"
-#include "lx_team.cuh"
+#include "lx_owner.cuh"
 
 namespace lx {
 
@@ -288,18 +288,12 @@ using namespace lx;
 // ================================================================================================ C ABI
 extern "C" {
 
-const char *lx_version(void) { return "lx3 0.2 sm_100a (team/chain/lane/group kernels, Lx<=6, La,Lb<=4)"; }
+const char *lx_version(void) { return "lx3 0.3 sm_100a (team/chain/owner/lane/group kernels, Lx<=6, La,Lb<=4)"; }
 
 const char *lx_kernel_family(int lx_, int la, int lb) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
-    {
-        const int ca = std::max(la, lb), cb = std::min(la, lb);
-        const bool wide = lx_ == 3 && ca == 2 && cb == 1;
-        const int tw = (ca + cb <= 4) ? team_size(lx_, ca, cb, wide ? 80 : 72) : 0;
-        if (tw > 0 && (lx_ <= 4 ? (ca + cb <= 2 || tw <= (wide ? 3 : 2)) : (ca + cb >= 1 && tw <= 3))) return "team";
-        if (chain_fits(lx_, ca, cb)) return "chain";
-    }
-    return lane_fits(std::max(la, lb), std::min(la, lb)) ? "lane" : "group";
+    static const char *names[] = {"team", "owner", "chain", "lane", "group"};
+    return names[class_family(lx_, std::max(la, lb), std::min(la, lb))];
 }
 
 const char *lx_strerror(int status) {

@@ -5,6 +5,7 @@
 #include <cstring>
 
 #include "lx_chain_kernel.cuh"
+#include "lx_owner.cuh"
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
@@ -15,33 +16,25 @@ namespace lx {
 
 // kernel family per class: team kernel where the chain targets of a warp fit its registers,
 // warp-specialised chain kernel for the other classes with La+Lb <= 4 and Lx <= 4, lane / group kernels beyond.
-// LX_FAMILY=team|chain|lane in the environment overrides the choice where the named family exists (tuning aid).
-#ifndef LX_TEAM_WMAX
-#define LX_TEAM_WMAX 2
-#endif
-#ifndef LX_TEAM_BUDGET
-#define LX_TEAM_BUDGET 72
-#endif
+// In builds with -DLX_TUNING (LX_EXTRA_NVCC=-DLX_TUNING) LX_FAMILY=team|chain|lane|owner in the environment overrides the
+// choice where the named family exists; regular builds compile one family per class.
+#ifdef LX_TUNING
 static int family_override() {
     static int v = -1;
     if (v < 0) {
         const char *e = std::getenv("LX_FAMILY");
-        v = !e ? 0 : (!std::strcmp(e, "team") ? 1 : (!std::strcmp(e, "chain") ? 2 : (!std::strcmp(e, "lane") ? 3 : 0)));
+        v = !e ? 0 : (!std::strcmp(e, "team") ? 1 : (!std::strcmp(e, "chain") ? 2 : (!std::strcmp(e, "lane") ? 3 : (!std::strcmp(e, "owner") ? 4 : 0))));
     }
     return v;
 }
+#endif
 
 template <int LX, int LA, int LB, int MODE>
 static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                                 const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                                 cudaStream_t stream) {
-    constexpr bool small = LA + LB <= 4 && LX <= LX_MAX_L_AUX;   // team: any Lx; the chain kernel has its own bound (Lx <= 4)
-    // (3|21) keeps all 13 targets in three warps with 80 accumulator doubles per lane: measured faster than the chain kernel
-    constexpr bool wide = LX == 3 && LA == 2 && LB == 1;
-    constexpr int TW = small ? team_size(LX, LA, LB, wide ? 80 : LX_TEAM_BUDGET) : 0;
-    // measured (B200): for Lx <= 4 the team kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets;
-    // for Lx = 5, 6 it beats the lane kernel while at most three warps hold the targets
-    constexpr bool has_team = TW > 0 && (LX <= 4 ? (LA + LB <= 2 || TW <= (wide ? 3 : LX_TEAM_WMAX)) : (LA + LB >= 1 && TW <= 3)), has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
+    constexpr int TW = team_width(LX, LA, LB);
+    constexpr bool has_team = TW > 0, has_chain = ChainCls<LX, LA, LB>::fits, has_lane = LaneCls<LX, LA, LB>::fits;
     if constexpr (MODE == 3) {
         // fused solid-harmonic aux functions: team kernel only; the caller falls back to Cartesian + lx_cart_to_pure
         if constexpr (has_team && LX >= 2)
@@ -51,7 +44,15 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         else
             return cudaErrorNotSupported;
     } else {
+    // Lx = 5, 6 at La+Lb <= 4: one owner warp per ket component (lx_owner.cuh) where the team kernel does not apply
+    constexpr bool has_owner = owner_fits(LX, LA, LB);
+#ifdef LX_TUNING
+    // tuning builds compile every family for every class; LX_FAMILY picks one at run time where it exists
     const int ov = family_override();
+    if constexpr (has_owner) {
+        if (ov == 4 || (ov == 0 && !has_team))
+            return owner_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    }
     if constexpr (has_team) {
         if (ov == 0 || ov == 1 || (ov == 2 && !has_chain) || (ov == 3 && !has_lane))
             return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
@@ -64,6 +65,18 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+#else
+    if constexpr (has_team)
+        return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else if constexpr (has_owner)
+        return owner_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else if constexpr (has_chain)
+        return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else if constexpr (has_lane)
+        return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else
+        return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+#endif
     }
 }
 

@@ -1,0 +1,382 @@
+// lx_owner.cuh — "owner kernel": the chain form of lx_chain.cuh with ONE OWNER PER KET COMPONENT, for high aux angular
+// momentum (Lx = 5, 6) at La+Lb <= 4.
+//
+// The resummed ket recurrence (lx_chain.cuh header; eq. 2 of the paper, plus the c−1 terms of reading G4)
+//
+//     [a0|c]^(0) = Σ_{n <= c/2}  β(c,n) (2ζc)^{−|n|} (2(γ+ζc))^{−|c−2n|} ( Π_i B_i^{c_i − 2n_i} Y_{|n|} )[a]
+//
+// is evaluated here per ket component c: a consumer warp (LANE = shell-set, 32 sets per batch) owns one c per pass, runs
+// the chains of ALL its partners n on the start vectors Y_p / a! (shared memory, written by the producer warps: one
+// warp per level p = 0..Lx/2) and sums them, weighted by the integers β, into one register accumulator — over the
+// partners and over the primitives (a5, "early contraction").  Compared with the team / chain kernels
+// (one chain per DISTINCT target (p, t), then a gather through shared memory) a level-p chain is run once per c that
+// needs it (119 chains instead of 50 targets for Lx = 6), but nothing is staged: the finished (e0|c) of the 32 sets is
+// in the owner's registers, goes through the HRR (a7, eq. 1) right there and leaves through a private
+// 32 × nc(La)nc(Lb) staging slot as a coalesced run (a8) or is digested (a9/a10).  Shared memory holds only
+// the start vectors (double-buffered over the primitive loop) and the staging slots, so that Lx = 5, 6 fit where the
+// (e0|c) region of the chain kernel (32 sets × nc(Lx) × NACC doubles) does not.
+#pragma once
+#include "lx_team.cuh"
+
+namespace lx {
+
+// does the class (La >= Lb) have an owner kernel?
+__host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
+    return LX >= 5 && LX <= LX_MAX_L_AUX && LA + LB == 4 && LB <= 2 && LA >= LB;
+}
+
+template <int LX, int LA, int LB>
+struct OwnCls {
+    static constexpr int E = LA + LB, NG = off(E + 1), NACC = NG - off(LA);
+    static constexpr int NXC = nc(LX), NA = nc(LA), NB = nc(LB), NAB = NA * NB, NINT = NXC * NAB;
+    static constexpr int NLEV = LX / 2 + 1;                       // levels p = 0..Lx/2, one producer warp each
+    // warps per block from the register budget of a consumer (chain copy NG + accumulator NACC doubles, plus scalars)
+    static constexpr int NW = E <= 2 ? 24 : (E == 3 ? 16 : 12);
+    // contracted batches (K > 1): warps [0, NWC) own one ket component per pass, warps [NWC, NW) produce
+    static constexpr int NWC = NW - NLEV;
+    static constexpr int NPASS = (NXC + NWC - 1) / NWC;
+    static constexpr int NCP = (NXC + NPASS - 1) / NPASS;         // ket components per pass (balanced over the passes)
+    static constexpr int SP = NAB | 1;                            // staging stride of a set (odd: conflict-free both ways)
+    static constexpr int UREC = NLEV * NG + 3 + NLEV;             // doubles per set of one start-vector buffer: u, r[3], ck[p]
+    static_assert(NWC >= 1 && NCP <= NWC, "consumer warps cover a pass");
+};
+
+// Batch header in shared memory (lane = set).
+struct OwnHdr {
+    double A[3][32], C[3][32], AB[3][32];
+    long long po[32];
+    int xo0[32], Kab[32], K[32], a[32], b[32], x[32], p[32];
+    int kmax;      // largest K of the batch (0: no live set)
+    int ready;     // the start vectors of this (K = 1) batch were made ahead, during the previous batch
+    int next_c;    // K = 1 batches: next ket component to hand out (warps take components dynamically)
+    int pad;
+};
+
+// Producer: start vectors Y_p / a! (a3, eq. 3) of primitive q for the 32 sets of the batch; warp `pw` makes level pw.
+// Buffer layout [UREC][32]: u[p][g], r[3] = 2γ(P−C), ck[p] = (1/(2(γ+ζc)))^{Lx−2p} (1/(2ζc))^p.
+template <int LX, int LA, int LB>
+__device__ __forceinline__ void owner_produce(double *__restrict__ ub, const OwnHdr *hd, int q, int pw, int lane,
+                                              const DevShells &aux, const PairData &pdat,
+                                              const double *__restrict__ boys_tab) {
+    using OC = OwnCls<LX, LA, LB>;
+    constexpr int E = OC::E, NG = OC::NG, NLEV = OC::NLEV;
+    const double A[3] = {hd->A[0][lane], hd->A[1][lane], hd->A[2][lane]};
+    const double C[3] = {hd->C[0][lane], hd->C[1][lane], hd->C[2][lane]};
+    const int Kab = hd->Kab[lane], K = hd->K[lane], xo0 = hd->xo0[lane];
+    const bool on = q < K;
+    const int qq = on ? q : 0;
+    const int kx = qq / Kab, ij = qq - kx * Kab;
+    const double zc = aux.zeta[xo0 + kx], cxc = on ? aux.coef[xo0 + kx] : 0.0;
+    const PrimRec R = prim_rec(pdat.pd + (hd->po[lane] + ij) * PD_STRIDE, zc, cxc, A, C);
+    static_for<0, NLEV>([&](auto ip) {
+        constexpr int p = decltype(ip)::value;
+        if (pw == p) {
+            constexpr int MLO = LX - 2 * p, MHI = LX - p + E;
+            double F[MHI - MLO + 1];
+            boys_range<MLO, MHI>(boys_tab, R.T, F);
+            double u[NG];
+            vrr1_level<LX, E, p, MLO>(R, F, u);
+            static_for<0, NG>([&](auto ig) { ub[(p * NG + decltype(ig)::value) * 32 + lane] = u[decltype(ig)::value]; });
+            ub[(NLEV * NG + 3 + p) * 32 + lane] = level_scale<LX - 2 * p, p>(R);
+            if constexpr (p == 0) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ub[(NLEV * NG + d) * 32 + lane] = R.r[d];
+            }
+        }
+    });
+}
+
+
+// One chain with RUN-TIME step counts (tx, ty, tz): the three step bodies are compile-time unrolled on the register
+// copy z of the start vector, the loops around them are not.  Every ket component and every partner runs this one piece
+// of code, so that the whole kernel stays resident in the instruction cache: with compile-time chains per component
+// (≈ 400 KB of SASS for Lx = 6, each instruction executed once per batch of a K = 1 class) the warps stalled on
+// instruction fetch most of the time (measured: "no instruction" 7.9 of 19 stall cycles per issue).
+template <int LA, int E>
+__device__ __forceinline__ void owner_chain(const double *__restrict__ zb, int lane, int tx, int ty, int tz, double rx,
+                                            double ry, double rz, double ck, double (&acc)[off(E + 1) - off(LA)]) {
+    constexpr int NG = off(E + 1), NACC = NG - off(LA);
+    double z[NG];
+    static_for<0, NG>([&](auto ig) { z[decltype(ig)::value] = zb[decltype(ig)::value * 32 + lane]; });
+#pragma unroll 1
+    for (int j = 0; j < tx; ++j) chain_step<0, 0, NG>(z, rx);
+#pragma unroll 1
+    for (int j = 0; j < ty; ++j) chain_step<1, 0, NG>(z, ry);
+#pragma unroll 1
+    for (int j = 0; j < tz; ++j) chain_step<2, 0, NG>(z, rz);
+    static_for<0, NACC>([&](auto ii) { acc[decltype(ii)::value] = fma(ck, z[off(LA) + decltype(ii)::value], acc[decltype(ii)::value]); });
+}
+
+// All partners n <= c/2 of ket component c (index within the shell, order G2) for one primitive: acc += Σ_n β(c,n) ck_|n| (...)
+template <int LX, int LA, int LB>
+__device__ __forceinline__ void owner_partners(int c, const double *__restrict__ ub, int lane,
+                                               double (&acc)[OwnCls<LX, LA, LB>::NACC]) {
+    using OC = OwnCls<LX, LA, LB>;
+    constexpr int E = OC::E, NG = OC::NG, NLEV = OC::NLEV;
+    int s = 0;
+    while ((s + 1) * (s + 2) / 2 <= c) ++s;                     // s = c_y + c_z
+    const int cz = c - s * (s + 1) / 2, cy = s - cz, cx = LX - s;
+    const double rx = ub[(NLEV * NG + 0) * 32 + lane], ry = ub[(NLEV * NG + 1) * 32 + lane], rz = ub[(NLEV * NG + 2) * 32 + lane];
+    // β(c,n) = Π_i c_i!/(n_i!(c_i−2n_i)!2^{n_i}) grows along an axis by (c_i−2n_i)(c_i−2n_i−1)/(2(n_i+1)): kept as exact small
+    // integers in double (no integer division in the loop)
+    auto grow = [](int ci, int ni) { return (double)((ci - 2 * ni) * (ci - 2 * ni - 1)) * (ni == 0 ? 0.5 : (ni == 1 ? 0.25 : 1.0 / 6.0)); };
+    double bx = 1.0;
+#pragma unroll 1
+    for (int nx = 0; 2 * nx <= cx; ++nx) {
+        double bxy = bx;
+#pragma unroll 1
+        for (int ny = 0; 2 * ny <= cy; ++ny) {
+            double beta = bxy;
+#pragma unroll 1
+            for (int nz = 0; 2 * nz <= cz; ++nz) {
+                const int p = nx + ny + nz;
+                const double ck = beta * ub[(NLEV * NG + 3 + p) * 32 + lane];
+                owner_chain<LA, E>(ub + (size_t)p * NG * 32, lane, cx - 2 * nx, cy - 2 * ny, cz - 2 * nz, rx, ry, rz, ck, acc);
+                beta *= grow(cz, nz);
+            }
+            bxy *= grow(cy, ny);
+        }
+        bx *= grow(cx, nx);
+    }
+}
+
+// a7 + a8/a9/a10 of one finished ket component: HRR in registers (eq. 1), then the 32 sets leave through
+// the warp's staging slot as one coalesced run per set (MODE 0), are contracted with D into γ (MODE 1) or added to the
+// warp's partial J sums (MODE 2; `first`: the slot holds nothing yet).
+template <int LX, int LA, int LB, int MODE>
+__device__ __forceinline__ void owner_finish(int c, const double (&acc)[OwnCls<LX, LA, LB>::NACC], const OwnHdr *hd,
+                                             double *__restrict__ stw, int lane, long long batch, const SetMap &map,
+                                             const DevShells &aux, const DevShells &prim, double *__restrict__ out, bool tr,
+                                             const DfArgs &df, bool first) {
+    using OC = OwnCls<LX, LA, LB>;
+    constexpr int NACC = OC::NACC, NXC = OC::NXC, NA = OC::NA, NB = OC::NB, NAB = OC::NAB, SP = OC::SP;
+    double H0[NACC];
+    static_for<0, NACC>([&](auto ii) {
+        constexpr int i = decltype(ii)::value;
+        H0[i] = acc[i] * (double)cart_fact(off(LA) + i);        // back from the u = f / a! basis (lx_chain.cuh)
+    });
+    const double AB[3] = {hd->AB[0][lane], hd->AB[1][lane], hd->AB[2][lane]};
+    if constexpr (MODE == 0) {
+        hrr_store<LA, LB>(H0, AB, stw + (size_t)lane * SP, tr);
+        __syncwarp();
+        const int nlive = (int)min((long long)32, map.nsets - batch * 32);
+        const int total = nlive * NAB;
+        double *o = out + (batch * 32 * NXC + c) * NAB;
+        for (int it = lane; it < total; it += 32) {
+            const int s = it / NAB, i = it - s * NAB;
+            o[(size_t)s * (NXC * NAB) + i] = stw[s * SP + i];
+        }
+        __syncwarp();
+    } else {
+        double fin[NAB];
+        hrr_store<LA, LB>(H0, AB, fin, false);
+        const bool live = hd->p[lane] >= 0;
+        const int xs = hd->x[lane];
+        if constexpr (MODE == 1) {
+            // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
+            if (live) {
+                const int sa = hd->a[lane], sb = hd->b[lane];
+                const double *Dab = df.D + (size_t)prim.bf_off[sa] * df.ld + prim.bf_off[sb];
+                double sum = 0.0;
+#pragma unroll
+                for (int ia = 0; ia < NA; ++ia)
+#pragma unroll
+                    for (int ib = 0; ib < NB; ++ib) sum = fma(fin[ia * NB + ib], __ldg(Dab + (size_t)ia * df.ld + ib), sum);
+                atomicAdd(df.out + aux.bf_off[xs] + c, (sa != sb ? 2.0 : 1.0) * sum);
+            }
+        } else {
+            // partial sums of this warp: JS[set][ab] += (c|ab) d[bf(X)+c]; reduced over warps and lanes at the end of the batch
+            const double dc = live ? __ldg(df.D + aux.bf_off[xs] + c) : 0.0;
+            double *js = stw + (size_t)lane * SP;
+#pragma unroll
+            for (int i = 0; i < NAB; ++i) js[i] = first ? fin[i] * dc : fma(fin[i], dc, js[i]);
+        }
+    }
+}
+
+template <int LX, int LA, int LB, int MODE>
+__global__ void __launch_bounds__(OwnCls<LX, LA, LB>::NW * 32, 1)
+owner_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const double *__restrict__ boys_tab,
+             double *__restrict__ out, int swapped, DfArgs df) {
+    using OC = OwnCls<LX, LA, LB>;
+    constexpr int NACC = OC::NACC, NXC = OC::NXC, NB = OC::NB, NAB = OC::NAB;
+    constexpr int NLEV = OC::NLEV, NW = OC::NW, NWC = OC::NWC, NPASS = OC::NPASS, NCP = OC::NCP, SP = OC::SP, UREC = OC::UREC;
+    constexpr unsigned FULL = 0xffffffffu;
+
+    extern __shared__ double smem[];
+    double *U = smem;                                            // [2][UREC][32]
+    double *ST = U + (size_t)2 * UREC * 32;                      // [NW][32][SP]: staging (MODE 0) / J partial sums (MODE 2)
+    OwnHdr *hd2 = reinterpret_cast<OwnHdr *>(ST + (size_t)NW * 32 * SP);   // two headers: the next batch is decoded ahead
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long nbatch = (map.nsets + 31) / 32;
+    const bool tr = MODE == 0 && swapped != 0;                   // mirrored class: the caller's order is [c][b][a]
+    double *stw = ST + (size_t)warp * 32 * SP;
+
+    // header of batch bb (one warp, lane = set); batches past the end decode as empty (kmax = 0)
+    auto decode = [&](long long bb, OwnHdr *h) {
+        const SetId sid = decode_set(map, bb * 32 + lane, swapped);
+        const int Kab = min(prim.K[sid.a] * prim.K[sid.b], pdat.kstride);
+        const int K = sid.live ? Kab * aux.K[sid.x] : 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double Ad = prim.center[3 * sid.a + d];
+            h->A[d][lane] = Ad;
+            h->C[d][lane] = aux.center[3 * sid.x + d];
+            h->AB[d][lane] = Ad - prim.center[3 * sid.b + d];
+        }
+        h->po[lane] = pdat.pd_off ? pdat.pd_off[sid.p] : (long long)sid.p * pdat.kstride;
+        h->xo0[lane] = aux.prim_off[sid.x];
+        h->Kab[lane] = Kab;
+        h->K[lane] = K;
+        h->a[lane] = sid.a;
+        h->b[lane] = sid.b;
+        h->x[lane] = sid.x;
+        h->p[lane] = sid.live ? sid.p : -1;
+        const int km = __reduce_max_sync(FULL, K);
+        if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; }
+    };
+    if (warp == NWC) decode(blockIdx.x, hd2);
+
+    int it = 0;
+    for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x, ++it) {
+        __syncthreads();                                         // the previous batch is finished; this batch's header is there
+        OwnHdr *hd = hd2 + (it & 1), *hn = hd2 + ((it + 1) & 1);
+        const int kmax = hd->kmax;
+        bool first = true;                                       // MODE 2: this warp's partial J sums are still empty
+
+        if (kmax <= 1) {
+            // ============ K = 1 batch: start vectors once, then every warp takes ket components until none is left ============
+            double *ub = U + (size_t)(it & 1) * UREC * 32;
+            if (!hd->ready) {                                    // not made ahead (first batch of the block, or after a K > 1 batch)
+                if (warp >= NWC) owner_produce<LX, LA, LB>(ub, hd, 0, warp - NWC, lane, aux, pdat, boys_tab);
+                __syncthreads();
+            }
+            if (warp >= NWC) {
+                // look ahead: header of the next batch and, if it is a K = 1 batch too, its start vectors into the idle buffer
+                if (warp == NWC) decode(batch + gridDim.x, hn);
+                named_sync(2, NLEV * 32);
+                if (hn->kmax == 1) {
+                    owner_produce<LX, LA, LB>(U + (size_t)((it + 1) & 1) * UREC * 32, hn, 0, warp - NWC, lane, aux, pdat, boys_tab);
+                    if (warp == NWC && lane == 0) hn->ready = 1;
+                }
+            }
+            while (true) {
+                int c = 0;
+                if (lane == 0) c = atomicAdd(&hd->next_c, 1);
+                c = __shfl_sync(FULL, c, 0);
+                if (c >= NXC) break;
+                double acc[NACC];
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+                owner_partners<LX, LA, LB>(c, ub, lane, acc);
+                owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
+                first = false;
+            }
+        } else {
+            // ============ contracted batch: passes over the ket components, the primitive loop inside each pass ===========
+            if (warp == NWC) decode(batch + gridDim.x, hn);
+#pragma unroll 1
+            for (int pass = 0; pass < NPASS; ++pass) {
+                const int c = pass * NCP + warp;
+                const bool has = warp < NCP && c < NXC;
+                if (warp >= NWC) owner_produce<LX, LA, LB>(U, hd, 0, warp - NWC, lane, aux, pdat, boys_tab);
+                named_sync(1, NW * 32);
+                double acc[NACC];
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+#pragma unroll 1
+                for (int q = 0; q < kmax; ++q) {
+                    if (warp >= NWC) {
+                        if (q + 1 < kmax) owner_produce<LX, LA, LB>(U + (size_t)((q + 1) & 1) * UREC * 32, hd, q + 1, warp - NWC, lane, aux, pdat, boys_tab);
+                    } else if (has) {
+                        owner_partners<LX, LA, LB>(c, U + (size_t)(q & 1) * UREC * 32, lane, acc);
+                    }
+                    named_sync(1, NW * 32);                      // primitive q is consumed, q + 1 is produced
+                }
+                if (has) {
+                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
+                    first = false;
+                }
+            }
+        }
+
+        if constexpr (MODE == 2) {
+            // a10: J[bf(a)+ia, bf(b)+ib] += Σ_X Σ_c (c|ab) d[bf(X)+c], mirrored: sum the warps' partial sums, then the lanes
+            // that share a shell pair (contiguous runs of the batch) by shuffles; one atomic per run and element
+            if (first) {
+                for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
+            }
+            __syncthreads();
+            const int pl_own = hd->p[lane];
+            const bool live = pl_own >= 0;
+            const unsigned livemask = __ballot_sync(FULL, live);
+            const int sa = hd->a[lane], sb = hd->b[lane];
+            for (int r = warp; r < NAB; r += NW) {
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) v += ST[((size_t)w * 32 + lane) * SP + r];
+                const int ia = r / NB, ib = r - ia * NB;
+                unsigned rest = livemask;
+                while (rest) {
+                    const int leader = __ffs(rest) - 1;
+                    const int pl = __shfl_sync(FULL, pl_own, leader);
+                    const unsigned grp = __ballot_sync(FULL, live && pl_own == pl) & rest;
+                    double sum = (grp >> lane) & 1u ? v : 0.0;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+                    if (lane == leader) {
+                        const size_t ra0 = prim.bf_off[sa], rb0 = prim.bf_off[sb];
+                        atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
+                        if (sa != sb) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
+                    }
+                    rest &= ~grp;
+                }
+            }
+        }
+    }
+}
+
+template <int LX, int LA, int LB, int MODE>
+cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
+                         const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
+                         cudaStream_t stream) {
+    using OC = OwnCls<LX, LA, LB>;
+    constexpr size_t smem = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr);
+    static_assert(smem <= 227 * 1024, "owner kernel: batch does not fit in shared memory");
+    auto kern = owner_kernel<LX, LA, LB, MODE>;
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
+    if (map.nsets <= 0) return cudaSuccess;
+    long long blocks = (map.nsets + 31) / 32;
+    if (blocks > (long long)num_sms) blocks = num_sms;
+    kern<<<(unsigned)blocks, OC::NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+    return cudaGetLastError();
+}
+
+// ---- kernel family of a class (La >= Lb), shared by the dispatcher (lx_inst.cu) and lx_kernel_family() ------------------
+#ifndef LX_TEAM_WMAX
+#define LX_TEAM_WMAX 2
+#endif
+#ifndef LX_TEAM_BUDGET
+#define LX_TEAM_BUDGET 72
+#endif
+enum { FAM_TEAM = 0, FAM_OWNER = 1, FAM_CHAIN = 2, FAM_LANE = 3, FAM_GROUP = 4 };
+// warps of the team kernel of a class, 0 = the class does not run on the team kernel.  Measured (B200): for Lx <= 4 the team
+// kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets ((3|21): three warps with 80 accumulator doubles
+// per lane); for Lx = 5, 6 while at most three warps hold the targets.
+__host__ __device__ constexpr int team_width(int LX, int LA, int LB) {
+    if (LA + LB > 4) return 0;
+    const bool wide = LX == 3 && LA == 2 && LB == 1;
+    const int tw = team_size(LX, LA, LB, wide ? 80 : LX_TEAM_BUDGET);
+    const bool ok = tw > 0 && (LX <= 4 ? (LA + LB <= 2 || tw <= (wide ? 3 : LX_TEAM_WMAX)) : (LA + LB >= 1 && tw <= 3));
+    return ok ? tw : 0;
+}
+__host__ __device__ constexpr int class_family(int LX, int LA, int LB) {
+    if (team_width(LX, LA, LB) > 0) return FAM_TEAM;
+    if (owner_fits(LX, LA, LB)) return FAM_OWNER;
+    if (chain_fits(LX, LA, LB)) return FAM_CHAIN;
+    return lane_fits(LA, LB) ? FAM_LANE : FAM_GROUP;
+}
+
+}  // namespace lx
