@@ -292,7 +292,7 @@ const char *lx_version(void) { return "lx3 0.3 sm_100a (team/chain/owner/lane/gr
 
 const char *lx_kernel_family(int lx_, int la, int lb) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
-    static const char *names[] = {"team", "owner", "chain", "lane", "group"};
+    static const char *names[] = {"team", "owner", "chain", "lane", "group", "slab"};
     return names[class_family(lx_, std::max(la, lb), std::min(la, lb))];
 }
 

@@ -5,7 +5,7 @@
 #include <cstring>
 
 #include "lx_chain_kernel.cuh"
-#include "lx_owner.cuh"
+#include "lx_slab.cuh"
 #include "lx_dispatch.h"
 
 #ifndef INST_LX
@@ -74,6 +74,8 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else if constexpr (has_lane)
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    else if constexpr (slab_fits(LX, LA, LB) && MODE == 0)
+        return slab_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
 #endif

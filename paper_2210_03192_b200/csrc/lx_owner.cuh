@@ -46,10 +46,11 @@ struct OwnHdr {
     double A[3][32], C[3][32], AB[3][32];
     long long po[32];
     int xo0[32], Kab[32], K[32], a[32], b[32], x[32], p[32];
+    int tr[32];    // slab kernel: the set is stored transposed ([c][b][a]: mirrored class, or roles exchanged for La = Lb)
     int kmax;      // largest K of the batch (0: no live set)
     int ready;     // the start vectors of this (K = 1) batch were made ahead, during the previous batch
     int next_c;    // K = 1 batches: next ket component to hand out (warps take components dynamically)
-    int pad;
+    int next_p;    // slab kernel: next producer work item
 };
 
 // Producer: start vectors Y_p / a! (a3, eq. 3) of primitive q for the 32 sets of the batch; warp `pw` makes level pw.
@@ -234,7 +235,7 @@ owner_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         h->x[lane] = sid.x;
         h->p[lane] = sid.live ? sid.p : -1;
         const int km = __reduce_max_sync(FULL, K);
-        if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; }
+        if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; h->next_p = 0; }
     };
     if (warp == NWC) decode(blockIdx.x, hd2);
 
@@ -361,7 +362,7 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
 #ifndef LX_TEAM_BUDGET
 #define LX_TEAM_BUDGET 72
 #endif
-enum { FAM_TEAM = 0, FAM_OWNER = 1, FAM_CHAIN = 2, FAM_LANE = 3, FAM_GROUP = 4 };
+enum { FAM_TEAM = 0, FAM_OWNER = 1, FAM_CHAIN = 2, FAM_LANE = 3, FAM_GROUP = 4, FAM_SLAB = 5 };
 // warps of the team kernel of a class, 0 = the class does not run on the team kernel.  Measured (B200): for Lx <= 4 the team
 // kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets ((3|21): three warps with 80 accumulator doubles
 // per lane); for Lx = 5, 6 while at most three warps hold the targets.
@@ -376,7 +377,8 @@ __host__ __device__ constexpr int class_family(int LX, int LA, int LB) {
     if (team_width(LX, LA, LB) > 0) return FAM_TEAM;
     if (owner_fits(LX, LA, LB)) return FAM_OWNER;
     if (chain_fits(LX, LA, LB)) return FAM_CHAIN;
-    return lane_fits(LA, LB) ? FAM_LANE : FAM_GROUP;
+    if (lane_fits(LA, LB)) return FAM_LANE;
+    return LA + LB >= 5 && LA + LB <= 6 ? FAM_SLAB : FAM_GROUP;   // slab kernel (lx_slab.cuh); the group kernel still serves its DF modes
 }
 
 }  // namespace lx

@@ -52,7 +52,7 @@ def test_workspace_bytes_and_family(lx):
     for lxa in range(7):
         for la in range(5):
             for lb in range(5):
-                assert lx.lx_kernel_family(lxa, la, lb) in ("team", "chain", "owner", "lane", "group")
+                assert lx.lx_kernel_family(lxa, la, lb) in ("team", "chain", "owner", "lane", "group", "slab")
                 assert lx.lx_kernel_family(lxa, la, lb) == lx.lx_kernel_family(lxa, lb, la)
 
 
