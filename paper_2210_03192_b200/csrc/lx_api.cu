@@ -485,7 +485,8 @@ int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shel
         if ((rc = lx_async_status()) != LX_OK) return rc;
     }
     if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kstride, pd, st)) != LX_OK) return rc;
-    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr};
+    // khint: the stride bounds K_a K_b; the aux contraction is not known on the host (aux shells are mostly uncontracted)
+    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr, kstride};
     PairData pdat{pd, nullptr, kstride};
     DfArgs df{nullptr, nullptr, 0};
     cudaError_t e = k_launch[0][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
@@ -521,7 +522,7 @@ int lx_eri3_batch_pure(int lx_, int la, int lb, const lx_shells_t *aux, const lx
     double *pd = reinterpret_cast<double *>(workspace);
     // fused path: level-0 chain targets + solid-harmonic projection in the epilogue (team kernel classes, Lx >= 2)
     if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kmax_pair, pd, st)) != LX_OK) return rc;
-    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr};
+    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr, kmax_pair};
     PairData pdat{pd, nullptr, kmax_pair};
     DfArgs df{g.solid[lx_], nullptr, 0};
     cudaError_t e = k_launch[3][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
@@ -643,7 +644,11 @@ int lx_schedule_create(const lx_shells_t *aux, const lx_shells_t *prim, const do
         long long po = 0;
         for (const P &p : ps) {
             const int la = prim->L[p.a], lb = prim->L[p.b];
-            if (s->pair_b.empty() || s->pair_b.back().la != la || s->pair_b.back().lb != lb) {
+            // one bucket per (La, Lb) and contraction class K_a K_b = 1 | 2 | 3-4 | 5-9 | >= 10: launches are nearly uniform in
+            // K, and K-aware kernel choices (lx_inst.cu) see a tight bound
+            auto kclass = [](int k) { return k <= 1 ? 0 : (k == 2 ? 1 : (k <= 4 ? 2 : (k <= 9 ? 3 : 4))); };
+            if (s->pair_b.empty() || s->pair_b.back().la != la || s->pair_b.back().lb != lb ||
+                kclass(s->pair_b.back().kmax) != kclass(p.kab)) {
                 s->pair_b.emplace_back();
                 s->pair_b.back().la = la;
                 s->pair_b.back().lb = lb;
@@ -731,7 +736,7 @@ static int df_run(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shell
     for (const auto &l : s->launches) {
         const auto &ab = s->aux_b[l.ab];
         const auto &pb = s->pair_b[l.pb];
-        SetMap map{l.nsets, (int)ab.ids.size(), (int)pb.q.size(), ab.d_ids, pb.d_pairs, l.d_cum};
+        SetMap map{l.nsets, (int)ab.ids.size(), (int)pb.q.size(), ab.d_ids, pb.d_pairs, l.d_cum, pb.kmax * ab.K};
         PairData pdat{pd, pb.d_pd_off, pb.kmax};
         cudaError_t e = k_launch[mode][ab.L](pb.la, pb.lb, map, daux, dprim, pdat, g.boys_tab, nullptr, 0, df, g.num_sms, st);
         g.launches++;

@@ -47,6 +47,7 @@ struct SetMap {
     const int32_t *x_list;     // aux shell ids
     const int32_t *pair_list;  // [npair][2] primary shell ids in CANONICAL order (L of first >= L of second)
     const long long *cum;      // [npair+1] or nullptr
+    int khint;                 // host-side upper bound of K_a K_b K_x over the launch where known (0 = unknown): picks K-aware kernels
 };
 
 // Primitive-pair data: per primitive pair PD_STRIDE doubles {γ, Px, Py, Pz, K_ij, 1/(2γ)},

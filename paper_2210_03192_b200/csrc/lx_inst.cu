@@ -66,15 +66,22 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
 #else
-    if constexpr (has_team)
+    if constexpr (has_owner) {
+        // La+Lb >= 3: always; La+Lb = 2: only where the launch is known to be weakly contracted (the team / lane kernels win
+        // at high K: their per-primitive work is one chain per distinct target, the owner's one per partner)
+        if (LA + LB >= 3 || (map.khint > 0 && map.khint <= OWNER_KMAX_E2))
+            return owner_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
+    }
+    constexpr bool owner_only = has_owner && LA + LB >= 3;
+    if constexpr (owner_only)
+        return cudaErrorUnknown;   // not reached
+    else if constexpr (has_team)
         return team_launch<LX, LA, LB, MODE, (TW > 0 ? TW : 1)>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
-    else if constexpr (has_owner)
-        return owner_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else if constexpr (has_chain)
         return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else if constexpr (has_lane)
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
-    else if constexpr (slab_fits(LX, LA, LB) && MODE == 0)
+    else if constexpr (slab_fits(LX, LA, LB))
         return slab_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);

@@ -22,7 +22,7 @@ namespace lx {
 
 // does the class (La >= Lb) have an owner kernel?
 __host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
-    return LX >= 5 && LX <= LX_MAX_L_AUX && LA + LB == 4 && LB <= 2 && LA >= LB;
+    return LX >= 5 && LX <= LX_MAX_L_AUX && LA + LB >= 2 && LA + LB <= 4 && LB <= 2 && LA >= LB;
 }
 
 template <int LX, int LA, int LB>
@@ -362,6 +362,7 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
 #ifndef LX_TEAM_BUDGET
 #define LX_TEAM_BUDGET 72
 #endif
+constexpr int OWNER_KMAX_E2 = 4;   // La+Lb = 2 classes run on the owner kernel up to this contraction degree (measured)
 enum { FAM_TEAM = 0, FAM_OWNER = 1, FAM_CHAIN = 2, FAM_LANE = 3, FAM_GROUP = 4, FAM_SLAB = 5 };
 // warps of the team kernel of a class, 0 = the class does not run on the team kernel.  Measured (B200): for Lx <= 4 the team
 // kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets ((3|21): three warps with 80 accumulator doubles
@@ -374,11 +375,11 @@ __host__ __device__ constexpr int team_width(int LX, int LA, int LB) {
     return ok ? tw : 0;
 }
 __host__ __device__ constexpr int class_family(int LX, int LA, int LB) {
+    if (owner_fits(LX, LA, LB)) return FAM_OWNER;   // La+Lb = 2: for launches known to have K <= OWNER_KMAX_E2, else team / lane
     if (team_width(LX, LA, LB) > 0) return FAM_TEAM;
-    if (owner_fits(LX, LA, LB)) return FAM_OWNER;
     if (chain_fits(LX, LA, LB)) return FAM_CHAIN;
     if (lane_fits(LA, LB)) return FAM_LANE;
-    return LA + LB >= 5 && LA + LB <= 6 ? FAM_SLAB : FAM_GROUP;   // slab kernel (lx_slab.cuh); the group kernel still serves its DF modes
+    return LX >= 3 && LA + LB >= 5 && LA + LB <= 6 ? FAM_SLAB : FAM_GROUP;   // slab kernel (lx_slab.cuh)
 }
 
 }  // namespace lx

@@ -178,10 +178,11 @@ __host__ __device__ constexpr SlabGroups slab_groups(int E) {
 }
 
 // a4/a5 for (ket component c, slab group G): all partners n <= c/2 of the kprim primitives in `ub` (buffers of UREC*NS
-// doubles), accumulated in registers; then (e0|c) = acc · a! of the group's slabs goes to the owner's E0 region.
+// doubles), accumulated in registers; then scale · (e0|c) = scale · acc · a! of the group's slabs goes to (add: is added to) the
+// owner's E0 region (scale = 1, or d_c when the team sums Σ_c d_c (e0|c) for the J digestion).
 template <int LX, int LA, int LB, int G>
 __device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *__restrict__ ub, int kprim,
-                                         double *__restrict__ e0w, int ls, bool add) {
+                                         double *__restrict__ e0w, int ls, bool add, double scale) {
     using SC = SlabCls<LX, LA, LB>;
     constexpr int E = SC::E, NG = SC::NG, NS = SC::NS;
     constexpr SlabGroups GR = slab_groups(E);
@@ -257,8 +258,8 @@ __device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *_
             static_for<0, d + 1>([&](auto iq) {
                 constexpr int q = decltype(iq)::value, i = ao + tsz(d) + q - T0;
                 constexpr double f = (double)ifact(S) * (double)ifact(d - q) * (double)ifact(q);
-                if (add) dst[(size_t)i * NS] += acc[i] * f;
-                else dst[(size_t)i * NS] = acc[i] * f;
+                if (add) dst[(size_t)i * NS] = fma(acc[i], f * scale, dst[(size_t)i * NS]);
+                else dst[(size_t)i * NS] = acc[i] * (f * scale);
             });
         });
     });
@@ -268,10 +269,14 @@ __device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *_
 // unrolled).  The x part of b is summed from the slabs S..S+b_x of the warp's (e0|c) region; the y and z parts are
 // up-shifting steps v[a] <- AB_i v[a] + v[a+1_i] on the band of in-slab degrees d0..d0+m (d0 = LA−S, m = LB−b_x) in
 // registers.  The rows (all b) of the NS sets go to the staging slot and leave as one contiguous run per set.
+// MODE 1 (a9): instead of the store the lane contracts its staged rows with the D block of its pair and returns the partial
+// sum Σ_{a: a_x = S} Σ_b (c|ab) D_ab.  MODE 2 (a10): e0w holds Σ_c d_c (e0|c) of the batch; the staged rows are the lane's J
+// contributions, which slab_j_reduce adds to J.
+struct SlabDf { const OwnHdr *hd; const int32_t *bf_off; DfArgs df; };
 template <int LX, int LA, int LB, int S, int MODE>
-__device__ __noinline__ void slab_hrr(const double *__restrict__ e0w, double *__restrict__ stw, const double (&AB)[3],
-                                         int c, int ls, int lane, long long batch, long long nsets,
-                                         double *__restrict__ out, const int *__restrict__ trs) {
+__device__ __noinline__ double slab_hrr(const double *__restrict__ e0w, double *__restrict__ stw, const double (&AB)[3],
+                                        int c, int ls, int lane, long long batch, long long nsets,
+                                        double *__restrict__ out, const int *__restrict__ trs, const SlabDf &sd) {
     using SC = SlabCls<LX, LA, LB>;
     constexpr int E = SC::E, NS = SC::NS, NA = SC::NA, NB = SC::NB, NAB = SC::NAB, NXC = SC::NXC;
     constexpr int D0 = LA - S, CH = (D0 + 1) * NB, SPS = SC::STG | 1;
@@ -351,7 +356,54 @@ __device__ __noinline__ void slab_hrr(const double *__restrict__ e0w, double *__
             dst += (size_t)SPT * (NXC * NAB);
         }
     }
+    double ret = 0.0;
+    if constexpr (MODE == 1) {
+        const OwnHdr *hd = sd.hd;
+        if (hd->p[ls] >= 0) {
+            const double *Dab = sd.df.D + (size_t)(sd.bf_off[hd->a[ls]] + tsz(D0)) * sd.df.ld + sd.bf_off[hd->b[ls]];
+#pragma unroll 1
+            for (int q = 0; q <= D0; ++q)
+#pragma unroll
+                for (int ib = 0; ib < NB; ++ib) ret = fma(strow[q * NB + ib], __ldg(Dab + (size_t)q * sd.df.ld + ib), ret);
+        }
+    }
     __syncwarp();
+    return ret;
+}
+
+// a10, last step: the rows a_x = S staged by slab_hrr<.., 2> are the sets' J contributions; warp `w` of `nw` takes the elements
+// i = w, w + nw, ..: the lanes that share a shell pair (contiguous runs of the batch) are summed by shuffles, one atomic per
+// run and element (mirrored for a != b).
+template <int LX, int LA, int LB, int S>
+__device__ __forceinline__ void slab_j_reduce(const double *__restrict__ strow, int w, int nw, int ls, int lane, const SlabDf &sd) {
+    using SC = SlabCls<LX, LA, LB>;
+    constexpr int NS = SC::NS, NB = SC::NB, D0 = LA - S, CH = (D0 + 1) * NB;
+    constexpr unsigned FULL = 0xffffffffu;
+    const OwnHdr *hd = sd.hd;
+    const int pl_own = lane < NS ? hd->p[ls] : -1;
+    const bool live = pl_own >= 0;
+    const unsigned livemask = __ballot_sync(FULL, live);
+    const int sa = hd->a[ls], sb = hd->b[ls];
+    const size_t ra0 = sd.bf_off[sa] + tsz(D0), rb0 = sd.bf_off[sb];
+#pragma unroll 1
+    for (int i = w; i < CH; i += nw) {
+        const double v = live ? strow[i] : 0.0;
+        const int q = i / NB, ib = i - q * NB;
+        unsigned rest = livemask;
+        while (rest) {                                          // warp-uniform loop over the runs of equal pairs
+            const int leader = __ffs(rest) - 1;
+            const int pl = __shfl_sync(FULL, pl_own, leader);
+            const unsigned grp = __ballot_sync(FULL, live && pl_own == pl) & rest;
+            double sum = (grp >> lane) & 1u ? v : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+            if (lane == leader) {
+                atomicAdd(sd.df.out + (ra0 + q) * sd.df.ld + rb0 + ib, sum);
+                if (sa != sb) atomicAdd(sd.df.out + (rb0 + ib) * sd.df.ld + ra0 + q, sum);
+            }
+            rest &= ~grp;
+        }
+    }
 }
 
 // Per-primitive scalars of the lane's set (as owner_produce) for primitive q of the batch in header h.
@@ -400,27 +452,34 @@ __host__ __device__ constexpr int snake(int k, int T) { return (k % (2 * T)) < T
 // the slab groups team member wt runs for ket component c
 template <int LX, int LA, int LB>
 __device__ __forceinline__ void slab_component_chains(int c, int wt, const double *__restrict__ ub, int kprim,
-                                                      double *__restrict__ e0t, int ls, bool add) {
+                                                      double *__restrict__ e0t, int ls, bool add, double scale) {
     constexpr int E = LA + LB, T = SlabCls<LX, LA, LB>::T;
     int s = 0;
     while ((s + 1) * (s + 2) / 2 <= c) ++s;
     const int cz = c - s * (s + 1) / 2, cy = s - cz, cx = LX - s;
     static_for<0, slab_groups(E).n>([&](auto ig) {
         constexpr int g = decltype(ig)::value;
-        if (wt == snake(g, T)) slab_chains<LX, LA, LB, g>(cx, cy, cz, ub, kprim, e0t, ls, add);
+        if (wt == snake(g, T)) slab_chains<LX, LA, LB, g>(cx, cy, cz, ub, kprim, e0t, ls, add, scale);
     });
 }
-// the rows (a_x = S) team member wt transfers and stores
+// the rows (a_x = S) team member wt transfers and stores (MODE 0) or contracts with D into γ (MODE 1, a9: PAPER.md:283, :365)
 template <int LX, int LA, int LB, int MODE>
 __device__ __forceinline__ void slab_component_finish(int c, int wt, const OwnHdr *hd, const double *__restrict__ e0t,
                                                       double *__restrict__ stw, int ls, int lane, long long batch,
-                                                      long long nsets, double *__restrict__ out) {
-    constexpr int T = SlabCls<LX, LA, LB>::T;
+                                                      long long nsets, double *__restrict__ out, const SlabDf &sd,
+                                                      const int32_t *__restrict__ aux_bf) {
+    constexpr int T = SlabCls<LX, LA, LB>::T, NS = SlabCls<LX, LA, LB>::NS;
     const double AB[3] = {hd->AB[0][ls], hd->AB[1][ls], hd->AB[2][ls]};
+    double part = 0.0;
     static_for<0, LA + 1>([&](auto is) {
         constexpr int S = decltype(is)::value;
-        if (wt == snake(S, T)) slab_hrr<LX, LA, LB, S, MODE>(e0t, stw, AB, c, ls, lane, batch, nsets, out, hd->tr);
+        if (wt == snake(S, T)) part += slab_hrr<LX, LA, LB, S, MODE>(e0t, stw, AB, c, ls, lane, batch, nsets, out, hd->tr, sd);
     });
+    if constexpr (MODE == 1) {
+        // γ[bf(X)+c] += f Σ_ab (c|ab) D_ab: every team member adds the rows it transferred
+        if (lane < NS && hd->p[ls] >= 0 && part != 0.0)
+            atomicAdd(sd.df.out + aux_bf[hd->x[ls]] + c, (hd->a[ls] != hd->b[ls] ? 2.0 : 1.0) * part);
+    }
 }
 
 template <int LX, int LA, int LB, int MODE>
@@ -452,7 +511,7 @@ slab_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
             // the VRR runs on the shell with the larger exponents (lx_common.cuh, shell_min_zeta): exchange the roles per set
             if (sid.live && shell_min_zeta(prim, sid.b) > shell_min_zeta(prim, sid.a)) {
                 const int t = sid.a; sid.a = sid.b; sid.b = t;
-                trs ^= 1;
+                if (MODE == 0) trs ^= 1;                         // the DF modes index D and J by the exchanged roles instead
             }
         }
         h->tr[ls] = trs;
@@ -484,6 +543,16 @@ slab_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
         OwnHdr *hd = hd2 + (it & 1), *hn = hd2 + ((it + 1) & 1);
         const int kmax = hd->kmax;
         if (warp == 0) decode(batch + gridDim.x, hn);
+        const SlabDf sd{hd, prim.bf_off, df};
+        // J digestion (MODE 2): the team's region sums G = Σ_c d_c (e0|c) over every component it takes; the HRR is linear and
+        // does not depend on c, so it runs once per batch on Σ_teams G (the step before the HRR is where the paper's J-engine
+        // contracts too)
+        const double dscale_on = (MODE == 2 && lane < NS && hd->p[ls] >= 0) ? 1.0 : 0.0;
+        const double *dvec = MODE == 2 ? df.D + aux.bf_off[hd->x[ls]] : nullptr;
+        if constexpr (MODE == 2) {
+            for (int i = wt * 32 + lane; i < NACC * NS; i += T * 32) e0t[i] = 0.0;
+            named_sync(1 + team, T * 32);
+        }
         if (kmax <= 1) {
             // ============ K = 1 batch: start vectors once (work items taken dynamically), then ket components dynamically ======
             while (true) {
@@ -499,36 +568,72 @@ slab_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
                 named_sync(1 + team, T * 32);
                 const int c = team_c[team];
                 if (c >= NXC) break;
-                slab_component_chains<LX, LA, LB>(c, wt, U, 1, e0t, ls, false);
-                named_sync(1 + team, T * 32);                    // (e0|c) of the team is complete
-                slab_component_finish<LX, LA, LB, MODE>(c, wt, hd, e0t, stw, ls, lane, batch, map.nsets, out);
-                named_sync(1 + team, T * 32);                    // ... and read
+                if constexpr (MODE == 2) {
+                    const double dc = dscale_on != 0.0 ? __ldg(dvec + c) : 0.0;
+                    slab_component_chains<LX, LA, LB>(c, wt, U, 1, e0t, ls, true, dc);
+                    named_sync(1 + team, T * 32);                // before the leader takes the next component
+                } else {
+                    slab_component_chains<LX, LA, LB>(c, wt, U, 1, e0t, ls, false, 1.0);
+                    named_sync(1 + team, T * 32);                // (e0|c) of the team is complete
+                    slab_component_finish<LX, LA, LB, MODE>(c, wt, hd, e0t, stw, ls, lane, batch, map.nsets, out, sd, aux.bf_off);
+                    named_sync(1 + team, T * 32);                // ... and read
+                }
             }
         } else {
-            // ============ contracted batch: passes of NW ket components; per pass one round per primitive ======================
+            // ============ contracted batch: passes of NTEAM ket components; per pass one round per primitive ===================
 #pragma unroll 1
             for (int c0 = 0; c0 < NXC; c0 += NTEAM) {
                 const int c = c0 + team;
+                double dc = 1.0;
+                if constexpr (MODE == 2) dc = (dscale_on != 0.0 && c < NXC) ? __ldg(dvec + c) : 0.0;
 #pragma unroll 1
                 for (int q = 0; q < kmax; ++q) {
                     __syncthreads();                             // the start vectors of the previous round are consumed
 #pragma unroll 1
                     for (int item = warp; item < NITEM; item += NW) slab_item<LX, LA, LB>(item, q, hd, U, ls, aux, pdat, boys_tab);
                     __syncthreads();
-                    if (c < NXC) slab_component_chains<LX, LA, LB>(c, wt, U, 1, e0t, ls, q > 0);
+                    if (c < NXC) slab_component_chains<LX, LA, LB>(c, wt, U, 1, e0t, ls, MODE == 2 || q > 0, dc);
                 }
-                __syncthreads();                                 // (e0|c) of every team is complete
-                if (c < NXC) slab_component_finish<LX, LA, LB, MODE>(c, wt, hd, e0t, stw, ls, lane, batch, map.nsets, out);
+                if constexpr (MODE != 2) {
+                    __syncthreads();                             // (e0|c) of every team is complete
+                    if (c < NXC) slab_component_finish<LX, LA, LB, MODE>(c, wt, hd, e0t, stw, ls, lane, batch, map.nsets, out, sd, aux.bf_off);
+                }
             }
+        }
+        if constexpr (MODE == 2) {
+            // a10: Σ over the teams, one HRR per set, then the lanes that share a shell pair are summed and added to J
+            __syncthreads();
+            for (int i = tid; i < NACC * NS; i += NW * 32) {
+                double g = E0[i];
+#pragma unroll
+                for (int t = 1; t < NTEAM; ++t) g += E0[(size_t)t * NACC * NS + i];
+                E0[i] = g;
+            }
+            __syncthreads();
+            const double AB[3] = {hd->AB[0][ls], hd->AB[1][ls], hd->AB[2][ls]};
+            static_for<0, (LA + NW) / NW>([&](auto ir) {           // rounds of NW row blocks: one staging slot per warp
+                constexpr int S0 = decltype(ir)::value * NW;
+                if constexpr (S0 > 0) __syncthreads();
+                static_for<S0, cmin(S0 + NW, LA + 1)>([&](auto is) {
+                    constexpr int S = decltype(is)::value;
+                    if (warp == S - S0) slab_hrr<LX, LA, LB, S, 2>(E0, stw, AB, 0, ls, lane, batch, map.nsets, out, hd->tr, sd);
+                });
+                __syncthreads();
+                static_for<S0, cmin(S0 + NW, LA + 1)>([&](auto is) {
+                    constexpr int S = decltype(is)::value;
+                    slab_j_reduce<LX, LA, LB, S>(ST + (size_t)(S - S0) * NS * SPS + (size_t)ls * SPS, warp, NW, ls, lane, sd);
+                });
+            });
         }
     }
 }
 
 // does the class (La >= Lb) run on the slab kernel?  Measured (B200, config 3, K = 1): (6|33) 32.5 -> 14.7 ms, (5|33) 15.6 ->
 // 9.3 ms against the group kernel; for La+Lb >= 7 the slabs (45 + 35 doubles for (4|44)) exceed the register file together
-// with the call frames and the group kernel is still faster (23.6 ms against 75 ms), so those classes stay there.
+// with the call frames and the group kernel is still faster (23.6 ms against 75 ms), so those classes stay there.  For
+// Lx <= 2 a batch has too few ket components to keep the teams busy (config 5 digestion: (0|32) 21 -> 29 ms): group kernel.
 __host__ __device__ constexpr bool slab_fits(int LX, int LA, int LB) {
-    return LA + LB >= 5 && LA + LB <= 6 && LA >= LB && LA <= LX_MAX_L_PRIM && LX <= LX_MAX_L_AUX;
+    return LX >= 3 && LA + LB >= 5 && LA + LB <= 6 && LA >= LB && LA <= LX_MAX_L_PRIM && LX <= LX_MAX_L_AUX;
 }
 
 template <int LX, int LA, int LB, int MODE>
