@@ -30,15 +30,24 @@ METRIC = "3-center integrals/sec (class sweep, config 2)"
 UNIT = "integrals/s"
 WORKLOAD = "configs[1]: 45 classes (Lx 0..4 | La,Lb 0..2), K_total=9, 1024 pairs x 256 aux per class"
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk/SM x 2 x sm_max_mhz
-HBM_PEAK_GBS = 6555.5                                   # MEASURED_PEAKS.json (driver-written copy bandwidth), BASELINE.md §2
+HBM_PEAK_GBS = 6555.5                                   # BASELINE.md §2 (MEASURED_PEAKS.json of round 1; overridden below if the file is there)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the tracked ncu --set full summaries under
 # profiles/ (never measured by this run: ncu is not available inside a timed bench); class -> (bytes, source file)
-NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): (1.071891e9 + 0.905e6, "profiles/r01_ncu_chain_4_2_2.md")}
+NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): (1.072485e9 + 1.226e6, "profiles/r02_ncu_chain_4_2_2.md (ncu --set full capture, round 2)")}
 # SURVEY.md §8(d) table, flops per shell-set for the classes it lists (K = 9 for config 2; config 3 as stated there)
 SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
                         (4, 1, 1): 29322, (4, 2, 2): 111054}
 SURVEY_FLOPS_CONFIG3 = {(6, 2, 2, 1): 43792, (5, 3, 3, 1): 70320, (6, 3, 3, 1): 116448, (4, 4, 4, 1): 93910,
                         (5, 2, 2, 5): 566418}
+
+
+def _measured_hbm():
+    """HBM peak of this pool's B200s as the driver measured it (MEASURED_PEAKS.json), else the BASELINE.md figure."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except Exception:
+        return HBM_PEAK_GBS, "BASELINE.md section 2 (MEASURED_PEAKS.json absent)"
 
 
 def ncart(l):
@@ -191,6 +200,7 @@ def bench_config3(lx, dev, costmodel):
     import torch
     res = {}
     buf = None
+    hbm, hbm_src = _measured_hbm()
     for cls in gen.CONFIG3_CLASSES:
         lxa, la, lb, k = cls
         cfg = gen.config3(lxa, la, lb, kprim=k)
@@ -208,7 +218,7 @@ def bench_config3(lx, dev, costmodel):
         call()
         call()
         ms = float(np.median(_time_calls(call, 5)))
-        t_hbm = 8.0 * nint / (HBM_PEAK_GBS * 1e9) * 1e3
+        t_hbm = 8.0 * nint / (hbm * 1e9) * 1e3
         fl_s, fl_m = SURVEY_FLOPS_CONFIG3[cls], costmodel.flops_per_set(lxa, la, lb, k * k)
         t_f64 = fl_s * nset / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
         floor = max(t_hbm, t_f64)
@@ -219,7 +229,7 @@ def bench_config3(lx, dev, costmodel):
             "frac_of_floor": floor / ms, "tflops_survey_count": fl_s * nset / (ms * 1e-3) / 1e12,
             "tflops_costmodel_count": fl_m * nset / (ms * 1e-3) / 1e12}
     return {"workload": "configs[2]: 4096 pairs x 128 aux shells per class, 256 atoms >= 1.5 bohr apart in a 15-bohr cube",
-            "peaks": {"hbm_gbs": HBM_PEAK_GBS, "fp64_tflops": FP64_NOMINAL_TFLOPS}, "classes": res}
+            "peaks": {"hbm_gbs": hbm, "hbm_source": hbm_src, "fp64_tflops": FP64_NOMINAL_TFLOPS}, "classes": res}
 
 
 def _df_model_flops(costmodel, aux, prim, pairs, qx, qp, tau):
@@ -311,6 +321,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-df", action="store_true", help="skip the DF-J (configs 4, 5) and solid-harmonic side measurements")
     ap.add_argument("--no-side", action="store_true", help="skip the config 1 / config 3 side measurements")
+    ap.add_argument("--c3", default="", help="profiling aid: run ONLY the given config-3 class, e.g. '6,3,3,1' (lx,la,lb,kprim), "
+                                             "three calls at full size (4096 pairs x 128 aux shells), print its time and exit")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -333,6 +345,17 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     lx.lx_init(local)
+
+    if args.c3:
+        lxa, la, lb, k = (int(v) for v in args.c3.split(","))
+        cfg = gen.config3(lxa, la, lb, kprim=k)
+        da, dp = lx.DeviceShells(cfg["aux"], dev), lx.DeviceShells(cfg["prim"], dev)
+        dx, dpr = torch.from_numpy(cfg["x_idx"]).to(dev), torch.from_numpy(cfg["pair_idx"]).to(dev)
+        out = torch.empty(4096 * 128 * ncart(lxa) * ncart(la) * ncart(lb), dtype=torch.float64, device=dev)
+        ws = torch.empty(lx.lx_eri3_workspace_bytes(lxa, la, lb, 128, 4096, k * k), dtype=torch.uint8, device=dev)
+        ms = _time_calls(lambda: lx.lx_eri3_batch(lxa, la, lb, da, dp, dx, dpr, out=out, workspace=ws, kmax=k * k), 3)
+        print(json.dumps({"config3_class": args.c3, "kernel": lx.lx_kernel_family(lxa, la, lb), "ms": ms}))
+        return
 
     # ---- inputs: one full config-2 batch per rank (weak scaling: independent shell-sets, no collective) --------
     classes = gen.CONFIG2_CLASSES
