@@ -223,7 +223,7 @@ def bench_config3(lx, dev, costmodel):
         t_f64 = fl_s * nset / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
         floor = max(t_hbm, t_f64)
         res[f"({lxa}|{la}{lb}) K={k * k}"] = {
-            "kernel": lx.lx_kernel_family(lxa, la, lb), "ms": ms, "integrals_per_s": nint / (ms * 1e-3),
+            "kernel": lx.lx_kernel_family_k(lxa, la, lb, k * k), "ms": ms, "integrals_per_s": nint / (ms * 1e-3),
             "shell_sets_per_s": nset / (ms * 1e-3), "hbm_write_gbs": 8.0 * nint / (ms * 1e-3) / 1e9,
             "floor_ms_hbm": t_hbm, "floor_ms_fp64_survey_flops": t_f64, "bound": "hbm" if t_hbm >= t_f64 else "alu",
             "frac_of_floor": floor / ms, "tflops_survey_count": fl_s * nset / (ms * 1e-3) / 1e12,
@@ -354,7 +354,7 @@ def main():
         out = torch.empty(4096 * 128 * ncart(lxa) * ncart(la) * ncart(lb), dtype=torch.float64, device=dev)
         ws = torch.empty(lx.lx_eri3_workspace_bytes(lxa, la, lb, 128, 4096, k * k), dtype=torch.uint8, device=dev)
         ms = _time_calls(lambda: lx.lx_eri3_batch(lxa, la, lb, da, dp, dx, dpr, out=out, workspace=ws, kmax=k * k), 3)
-        print(json.dumps({"config3_class": args.c3, "kernel": lx.lx_kernel_family(lxa, la, lb), "ms": ms}))
+        print(json.dumps({"config3_class": args.c3, "kernel": lx.lx_kernel_family_k(lxa, la, lb, k * k), "ms": ms}))
         return
 
     # ---- inputs: one full config-2 batch per rank (weak scaling: independent shell-sets, no collective) --------
@@ -504,7 +504,7 @@ def main():
         fl_survey = SURVEY_FLOPS_PER_SET.get(canon)
         t_top = class_ms[i_top] * 1e-3
         achieved = fl_set * nsets / t_top / 1e12
-        roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family(*canon)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
+        roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family_k(*canon, 9)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
                     "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(canon, (None, None))[0],
                     "traffic_source": NCU_DRAM_BYTES_PER_LAUNCH.get(canon, (None, "no ncu capture of this class under profiles/"))[1],

@@ -192,10 +192,15 @@ size_t lx_eri3_pure_workspace_bytes(int lx, int la, int lb, int nx, int npair, i
 int lx_solid_matrix(int l, double *matrix_host);
 
 /* Which kernel template serves a class: "team" (register-only chain form, lx_team.cuh), "chain" (warp-specialised
- * chain form, lx_chain_kernel.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
- * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only.  The environment
- * variable LX_FAMILY=team|chain|lane (read once) forces the named family where a class has it: a tuning aid. */
+ * chain form, lx_chain_kernel.cuh), "owner" (one owner warp per ket component, lx_owner.cuh), "slab" (the same with the bra
+ * vector cut into slabs, lx_slab.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
+ * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only.
+ * Some classes have two families and choose by the contraction degree of the launch ("K-aware
+ * dispatch"): lx_kernel_family_k takes the bound K_a K_b K_x the caller knows for the launch (what lx_eri3_batch derives from
+ * its K stride, the DF schedule from its buckets); kmax <= 0 = unknown.  lx_kernel_family(lx, la, lb) is the unknown case.
+ * Builds with -DLX_TUNING read LX_FAMILY=team|chain|lane|owner once and force the named family where a class has it. */
 const char *lx_kernel_family(int lx, int la, int lb);
+const char *lx_kernel_family_k(int lx, int la, int lb, int kmax);
 
 /* Number of kernel launches the library has issued since lx_init (for the bench's `gpu_launches` claim). */
 int64_t lx_launch_count(void);

@@ -290,11 +290,12 @@ extern "C" {
 
 const char *lx_version(void) { return "lx3 0.3 sm_100a (team/chain/owner/lane/group kernels, Lx<=6, La,Lb<=4)"; }
 
-const char *lx_kernel_family(int lx_, int la, int lb) {
+const char *lx_kernel_family_k(int lx_, int la, int lb, int kmax) {
     if (!(lx_ >= 0 && lx_ <= LX_MAX_L_AUX && la >= 0 && la <= LX_MAX_L_PRIM && lb >= 0 && lb <= LX_MAX_L_PRIM)) return "";
     static const char *names[] = {"team", "owner", "chain", "lane", "group", "slab"};
-    return names[class_family(lx_, std::max(la, lb), std::min(la, lb))];
+    return names[class_family(lx_, std::max(la, lb), std::min(la, lb), kmax)];
 }
+const char *lx_kernel_family(int lx_, int la, int lb) { return lx_kernel_family_k(lx_, la, lb, 0); }
 
 const char *lx_strerror(int status) {
     switch (status) {

@@ -45,7 +45,7 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
             return cudaErrorNotSupported;
     } else {
     // Lx = 5, 6 at La+Lb <= 4: one owner warp per ket component (lx_owner.cuh) where the team kernel does not apply
-    constexpr bool has_owner = owner_fits(LX, LA, LB);
+    constexpr bool has_owner = owner_fits(LX, LA, LB) && (LX >= 5 || !has_team);
 #ifdef LX_TUNING
     // tuning builds compile every family for every class; LX_FAMILY picks one at run time where it exists
     const int ov = family_override();
@@ -67,12 +67,12 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
 #else
     if constexpr (has_owner) {
-        // La+Lb >= 3: always; La+Lb = 2: only where the launch is known to be weakly contracted (the team / lane kernels win
-        // at high K: their per-primitive work is one chain per distinct target, the owner's one per partner)
-        if (LA + LB >= 3 || (map.khint > 0 && map.khint <= OWNER_KMAX_E2))
+        // weakly contracted launches (and every launch of the Lx = 5, 6 classes with La+Lb >= 3): the team / chain / lane kernels win
+        // at high K, where their per-primitive work (one chain per distinct target, the owner's: one per partner) decides
+        if (owner_kmax(LX, LA, LB) == (1 << 30) || (map.khint > 0 && map.khint <= owner_kmax(LX, LA, LB)))
             return owner_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     }
-    constexpr bool owner_only = has_owner && LA + LB >= 3;
+    constexpr bool owner_only = has_owner && owner_kmax(LX, LA, LB) == (1 << 30);
     if constexpr (owner_only)
         return cudaErrorUnknown;   // not reached
     else if constexpr (has_team)
@@ -81,7 +81,7 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
         return chain_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else if constexpr (has_lane)
         return lane_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
-    else if constexpr (slab_fits(LX, LA, LB))
+    else if constexpr (slab_fits(LX, LA, LB) || (MODE == 1 && LA == 3 && LB == 3 && LX >= 1))   // (1|33), (2|33) γ: 20 -> 6, 27 -> 11 ms (config 5)
         return slab_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);
     else
         return group_launch<LX, LA, LB, MODE>(map, aux, prim, pdat, boys_tab, out, swapped, df, num_sms, stream);

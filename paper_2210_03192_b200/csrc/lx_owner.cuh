@@ -16,13 +16,22 @@
 // the start vectors (double-buffered over the primitive loop) and the staging slots, so that Lx = 5, 6 fit where the
 // (e0|c) region of the chain kernel (32 sets × nc(Lx) × NACC doubles) does not.
 #pragma once
+#include <cstdlib>
+
 #include "lx_team.cuh"
 
 namespace lx {
 
-// does the class (La >= Lb) have an owner kernel?
+// does the class (La >= Lb) have an owner kernel?  Lx = 5, 6: La+Lb = 2..4.  Lx = 3, 4: the classes of the chain kernel
+// (La+Lb = 3, 4 where the team kernel does not apply), for weakly contracted launches only (owner_kmax).
 __host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
-    return LX >= 5 && LX <= LX_MAX_L_AUX && LA + LB >= 2 && LA + LB <= 4 && LB <= 2 && LA >= LB;
+    return LX >= 3 && LX <= LX_MAX_L_AUX && (LA + LB >= (LX >= 5 ? 2 : 3)) && LA + LB <= 4 && LB <= 2 && LA >= LB;
+}
+// largest contraction degree K_a K_b K_x (as known on the host, SetMap.khint) for which the owner kernel is chosen; measured on
+// config 5 (K = 1..4: (3|31) 41 -> 17 ms, (4|31) 43 -> 20 ms, (3|22) 26 -> 14 ms against the chain kernel) and config 2 (K = 9:
+// the chain / team kernels win for Lx <= 4, the owner kernel for Lx = 5, 6)
+__host__ __device__ constexpr int owner_kmax(int LX, int LA, int LB) {
+    return LX >= 5 ? (LA + LB >= 3 ? (1 << 30) : 4) : 4;
 }
 
 template <int LX, int LA, int LB>
@@ -338,19 +347,231 @@ owner_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
     }
 }
 
+// ---- owner kernel, resident form ------------------------------------------------------------------------------------------
+// For weakly contracted launches the start vectors of ALL primitives of a batch fit shared memory (NSLOT buffers), and
+// usually those of several batches do.  A block then takes up to OWN2_MAXB batches per round: every warp helps to make the
+// start vectors (work items (batch, primitive, level), handed out dynamically), and after one block barrier every warp owns
+// ket components of "its" batch (warp mod number of batches) with the primitive loop INSIDE the partner sums — no pass
+// structure, no barrier per primitive, no idle producer warps, and enough components per round for every warp even at
+// Lx = 3, 4 (10 / 15 components per batch).  A batch with more primitives than buffers runs in chunks of NSLOT primitives.
+constexpr int OWN2_MAXB = 4;
+struct Own2Ctl { int nb, tot, next_p, pad; int slot0[OWN2_MAXB + 1]; };
+template <int LX, int LA, int LB, int MODE>
+struct Own2Cls {
+    using OC = OwnCls<LX, LA, LB>;
+    static constexpr int UB = OC::UREC * 32;                              // doubles per start-vector buffer
+    static constexpr int STW = MODE == 1 ? 0 : 32 * OC::SP;               // staging (MODE 0) / J partial sums (MODE 2) per warp
+    static constexpr int fixed = OC::NW * STW * 8 + OWN2_MAXB * (int)sizeof(OwnHdr) + (int)sizeof(Own2Ctl) + 64;
+    static constexpr int NSLOT = cmin(16, (222 * 1024 - fixed) / (UB * 8));
+    static constexpr size_t smem = (size_t)fixed + (size_t)NSLOT * UB * 8;
+    static_assert(NSLOT >= 1, "owner kernel: no room for a start-vector buffer");
+};
+
+template <int LX, int LA, int LB, int MODE>
+__global__ void __launch_bounds__(OwnCls<LX, LA, LB>::NW * 32, 1)
+owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const double *__restrict__ boys_tab,
+              double *__restrict__ out, int swapped, DfArgs df) {
+    using OC = OwnCls<LX, LA, LB>;
+    using O2 = Own2Cls<LX, LA, LB, MODE>;
+    constexpr int NACC = OC::NACC, NXC = OC::NXC, NB = OC::NB, NAB = OC::NAB, NLEV = OC::NLEV, NW = OC::NW, SP = OC::SP;
+    constexpr int UB = O2::UB, NSLOT = O2::NSLOT, STW = O2::STW;
+    constexpr unsigned FULL = 0xffffffffu;
+
+    extern __shared__ double smem[];
+    double *U = smem;                                            // [NSLOT][UREC][32]
+    double *ST = U + (size_t)NSLOT * UB;                         // [NW][STW]
+    OwnHdr *hdr = reinterpret_cast<OwnHdr *>(ST + (size_t)NW * STW);
+    Own2Ctl *ctl = reinterpret_cast<Own2Ctl *>(hdr + OWN2_MAXB);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long nbatch = (map.nsets + 31) / 32, G = gridDim.x;
+    const bool tr = MODE == 0 && swapped != 0;
+    double *stw = ST + (size_t)warp * STW;
+
+    auto decode = [&](long long bb, OwnHdr *h) {
+        const SetId sid = decode_set(map, bb * 32 + lane, swapped);
+        const int Kab = min(prim.K[sid.a] * prim.K[sid.b], pdat.kstride);
+        const int K = sid.live ? Kab * aux.K[sid.x] : 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double Ad = prim.center[3 * sid.a + d];
+            h->A[d][lane] = Ad;
+            h->C[d][lane] = aux.center[3 * sid.x + d];
+            h->AB[d][lane] = Ad - prim.center[3 * sid.b + d];
+        }
+        h->po[lane] = pdat.pd_off ? pdat.pd_off[sid.p] : (long long)sid.p * pdat.kstride;
+        h->xo0[lane] = aux.prim_off[sid.x];
+        h->Kab[lane] = Kab;
+        h->K[lane] = K;
+        h->a[lane] = sid.a;
+        h->b[lane] = sid.b;
+        h->x[lane] = sid.x;
+        h->p[lane] = sid.live ? sid.p : -1;
+        const int km = __reduce_max_sync(FULL, K);
+        if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; h->next_p = 0; }
+    };
+    // a10 for the batch of header h: sum the partial J sums of the warps w = w0, w0 + dw, .. then the lanes that share a pair
+    auto j_reduce = [&](const OwnHdr *h, int w0, int dw) {
+        const int pl_own = h->p[lane];
+        const bool live = pl_own >= 0;
+        const unsigned livemask = __ballot_sync(FULL, live);
+        const int sa = h->a[lane], sb = h->b[lane];
+        for (int r = warp; r < NAB; r += NW) {
+            double v = 0.0;
+            for (int w = w0; w < NW; w += dw) v += ST[(size_t)w * STW + (size_t)lane * SP + r];
+            const int ia = r / NB, ib = r - ia * NB;
+            unsigned rest = livemask;
+            while (rest) {
+                const int leader = __ffs(rest) - 1;
+                const int pl = __shfl_sync(FULL, pl_own, leader);
+                const unsigned grp = __ballot_sync(FULL, live && pl_own == pl) & rest;
+                double sum = (grp >> lane) & 1u ? v : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+                if (lane == leader) {
+                    const size_t ra0 = prim.bf_off[sa], rb0 = prim.bf_off[sb];
+                    atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
+                    if (sa != sb) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
+                }
+                rest &= ~grp;
+            }
+        }
+    };
+
+    long long base = blockIdx.x;
+    while (base < nbatch) {
+        __syncthreads();                                         // the previous round is finished
+        if (warp < OWN2_MAXB) decode(base + warp * G, hdr + warp);
+        __syncthreads();
+        if (tid == 0) {
+            // plan of the round: as many of the next batches as have all their primitives resident
+            int nb = 0, tot = 0;
+            for (int i = 0; i < OWN2_MAXB; ++i) {
+                const int k = hdr[i].kmax;
+                if (k <= 0 || tot + k > NSLOT) break;
+                ctl->slot0[i] = tot;
+                tot += k;
+                ++nb;
+            }
+            ctl->slot0[nb] = tot;
+            ctl->nb = nb;
+            ctl->tot = tot;
+            ctl->next_p = 0;
+        }
+        __syncthreads();
+        const int nb = ctl->nb;
+        bool first = true;                                       // MODE 2: this warp's partial J sums are still empty
+        if (nb > 0) {
+            // ---- start vectors: work items (slot = (batch, primitive), level) ---------------------------------------------------
+            const int nitem = ctl->tot * NLEV;
+            while (true) {
+                int item = 0;
+                if (lane == 0) item = atomicAdd(&ctl->next_p, 1);
+                item = __shfl_sync(FULL, item, 0);
+                if (item >= nitem) break;
+                const int sq = item / NLEV, lev = item - sq * NLEV;
+                int i = 0;
+                while (i + 1 < nb && ctl->slot0[i + 1] <= sq) ++i;
+                owner_produce<LX, LA, LB>(U + (size_t)sq * UB, hdr + i, sq - ctl->slot0[i], lev, lane, aux, pdat, boys_tab);
+            }
+            __syncthreads();
+            // ---- ket components of this warp's batch ------------------------------------------------------------------------------
+            const int ib_ = warp % nb;
+            OwnHdr *hd = hdr + ib_;
+            const int kq = hd->kmax;
+            const double *ub0 = U + (size_t)ctl->slot0[ib_] * UB;
+            const long long batch = base + ib_ * G;
+            while (true) {
+                int c = 0;
+                if (lane == 0) c = atomicAdd(&hd->next_c, 1);
+                c = __shfl_sync(FULL, c, 0);
+                if (c >= NXC) break;
+                double acc[NACC];
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+#pragma unroll 1
+                for (int q = 0; q < kq; ++q) owner_partners<LX, LA, LB>(c, ub0 + (size_t)q * UB, lane, acc);
+                owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
+                first = false;
+            }
+            if constexpr (MODE == 2) {
+                if (first) {
+                    for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
+                }
+                __syncthreads();
+                for (int i = 0; i < nb; ++i) j_reduce(hdr + i, i, nb);
+            }
+            base += (long long)nb * G;
+        } else {
+            // ---- one batch with more primitives than buffers: chunks of NSLOT primitives, one ket component per warp and pass ------
+            OwnHdr *hd = hdr;
+            const int kmax = hd->kmax;
+#pragma unroll 1
+            for (int c0 = 0; c0 < NXC; c0 += NW) {
+                const int c = c0 + warp;
+                double acc[NACC];
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+#pragma unroll 1
+                for (int q0 = 0; q0 < kmax; q0 += NSLOT) {
+                    const int nq = min(NSLOT, kmax - q0);
+                    __syncthreads();                             // the previous chunk is consumed
+#pragma unroll 1
+                    for (int item = warp; item < nq * NLEV; item += NW) {
+                        const int sq = item / NLEV, lev = item - sq * NLEV;
+                        owner_produce<LX, LA, LB>(U + (size_t)sq * UB, hd, q0 + sq, lev, lane, aux, pdat, boys_tab);
+                    }
+                    __syncthreads();
+                    if (c < NXC) {
+#pragma unroll 1
+                        for (int q = 0; q < nq; ++q) owner_partners<LX, LA, LB>(c, U + (size_t)q * UB, lane, acc);
+                    }
+                }
+                if (c < NXC) {
+                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df, first);
+                    first = false;
+                }
+            }
+            if constexpr (MODE == 2) {
+                if (first) {
+                    for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
+                }
+                __syncthreads();
+                j_reduce(hd, 0, 1);
+            }
+            base += G;
+        }
+    }
+}
+
+// The resident form serves every launch whose K bound fits its buffers, except K = 1 launches of the Lx = 5, 6 classes, where
+// the look-ahead form above (start vectors of the next batch made during the current one) measured faster (LX_OWNER2=0|1 in the
+// environment forces one form: tuning aid).
 template <int LX, int LA, int LB, int MODE>
 cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                          const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
                          cudaStream_t stream) {
     using OC = OwnCls<LX, LA, LB>;
+    using O2 = Own2Cls<LX, LA, LB, MODE>;
+    if (map.nsets <= 0) return cudaSuccess;
+    long long blocks = (map.nsets + 31) / 32;
+    if (blocks > (long long)num_sms) blocks = num_sms;
+    static const int force = []() { const char *e = std::getenv("LX_OWNER2"); return e ? (e[0] == '1' ? 1 : 0) : -1; }();
+    bool resident = map.khint > 0 && map.khint <= O2::NSLOT && (LX <= 4 || map.khint > 1);
+    if (force >= 0) resident = force == 1;
+    if (resident) {
+        static_assert(O2::smem <= 227 * 1024, "owner kernel (resident form): does not fit in shared memory");
+        auto kern = owner2_kernel<LX, LA, LB, MODE>;
+        static std::atomic<unsigned long long> configured{0};
+        if (cudaError_t e = ensure_dyn_smem(kern, O2::smem, configured); e != cudaSuccess) return e;
+        kern<<<(unsigned)blocks, OC::NW * 32, O2::smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+        return cudaGetLastError();
+    }
     constexpr size_t smem = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr);
     static_assert(smem <= 227 * 1024, "owner kernel: batch does not fit in shared memory");
     auto kern = owner_kernel<LX, LA, LB, MODE>;
     static std::atomic<unsigned long long> configured{0};
     if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
-    if (map.nsets <= 0) return cudaSuccess;
-    long long blocks = (map.nsets + 31) / 32;
-    if (blocks > (long long)num_sms) blocks = num_sms;
     kern<<<(unsigned)blocks, OC::NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
     return cudaGetLastError();
 }
@@ -362,7 +583,6 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
 #ifndef LX_TEAM_BUDGET
 #define LX_TEAM_BUDGET 72
 #endif
-constexpr int OWNER_KMAX_E2 = 4;   // La+Lb = 2 classes run on the owner kernel up to this contraction degree (measured)
 enum { FAM_TEAM = 0, FAM_OWNER = 1, FAM_CHAIN = 2, FAM_LANE = 3, FAM_GROUP = 4, FAM_SLAB = 5 };
 // warps of the team kernel of a class, 0 = the class does not run on the team kernel.  Measured (B200): for Lx <= 4 the team
 // kernel wins for La+Lb <= 2 and wherever one or two warps hold all targets ((3|21): three warps with 80 accumulator doubles
@@ -374,8 +594,11 @@ __host__ __device__ constexpr int team_width(int LX, int LA, int LB) {
     const bool ok = tw > 0 && (LX <= 4 ? (LA + LB <= 2 || tw <= (wide ? 3 : LX_TEAM_WMAX)) : (LA + LB >= 1 && tw <= 3));
     return ok ? tw : 0;
 }
-__host__ __device__ constexpr int class_family(int LX, int LA, int LB) {
-    if (owner_fits(LX, LA, LB)) return FAM_OWNER;   // La+Lb = 2: for launches known to have K <= OWNER_KMAX_E2, else team / lane
+// khint: host-side bound of K_a K_b K_x of the launch, <= 0 = unknown (SetMap.khint)
+__host__ __device__ constexpr int class_family(int LX, int LA, int LB, int khint) {
+    if (owner_fits(LX, LA, LB) && (LX >= 5 || team_width(LX, LA, LB) == 0) &&
+        (owner_kmax(LX, LA, LB) == (1 << 30) || (khint > 0 && khint <= owner_kmax(LX, LA, LB))))
+        return FAM_OWNER;
     if (team_width(LX, LA, LB) > 0) return FAM_TEAM;
     if (chain_fits(LX, LA, LB)) return FAM_CHAIN;
     if (lane_fits(LA, LB)) return FAM_LANE;

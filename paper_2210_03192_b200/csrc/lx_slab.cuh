@@ -633,7 +633,7 @@ slab_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
 // with the call frames and the group kernel is still faster (23.6 ms against 75 ms), so those classes stay there.  For
 // Lx <= 2 a batch has too few ket components to keep the teams busy (config 5 digestion: (0|32) 21 -> 29 ms): group kernel.
 __host__ __device__ constexpr bool slab_fits(int LX, int LA, int LB) {
-    return LX >= 3 && LA + LB >= 5 && LA + LB <= 6 && LA >= LB && LA <= LX_MAX_L_PRIM && LX <= LX_MAX_L_AUX;
+    return LX >= 3 && LA + LB >= 5 && LA + LB <= 6 && LA >= LB && LA <= LX_MAX_L_PRIM && LX <= LX_MAX_L_AUX;   // + (1,2|33) in the γ mode, lx_inst.cu
 }
 
 template <int LX, int LA, int LB, int MODE>

@@ -22,7 +22,7 @@ LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
-           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family",
+           "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family", "lx_kernel_family_k",
            "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status",
            "lx_schwarz_aux_host", "lx_schwarz_pair_host"]
 
@@ -36,6 +36,8 @@ _lib.lx_strerror.restype = C.c_char_p
 _lib.lx_version.restype = C.c_char_p
 _lib.lx_kernel_family.restype = C.c_char_p
 _lib.lx_kernel_family.argtypes = [C.c_int] * 3
+_lib.lx_kernel_family_k.restype = C.c_char_p
+_lib.lx_kernel_family_k.argtypes = [C.c_int] * 4
 _lib.lx_eri3_workspace_bytes.restype = C.c_size_t
 _lib.lx_df_workspace_bytes.restype = C.c_size_t
 _lib.lx_df_workspace_bytes.argtypes = [C.c_void_p]
@@ -86,6 +88,10 @@ def lx_version():
 
 def lx_kernel_family(lx, la, lb):
     return _lib.lx_kernel_family(lx, la, lb).decode()
+
+
+def lx_kernel_family_k(lx, la, lb, kmax):
+    return _lib.lx_kernel_family_k(lx, la, lb, kmax).decode()
 
 
 def lx_strerror(status):

@@ -254,7 +254,7 @@ def test_config2_full_size_sampled(lx, oracle, lxa):
 
 def test_kernel_families_cover_config2(lx):
     """Every class of the class sweep runs on one of the register-resident families (no silent fallback)."""
-    fams = {c: lx.lx_kernel_family(*c) for c in gen.CONFIG2_CLASSES}
+    fams = {c: lx.lx_kernel_family_k(*c, 9) for c in gen.CONFIG2_CLASSES}      # config 2: K_a K_b K_x = 9
     assert set(fams.values()) <= {"team", "chain"}, fams
     assert fams[(4, 2, 2)] == "chain" and fams[(2, 1, 1)] == "team"
 
@@ -325,7 +325,7 @@ def test_config3_full_config_sampled(lx, oracle, cls):
     ref = oracle.eri3_batch(lxa, la, lb, cfg["aux"], cfg["prim"], cfg["x_idx"][xs], cfg["pair_idx"][ps])
     scale = np.max(np.abs(ref))
     ratio = np.max(np.abs(sub - ref)) / scale
-    print(f"config 3 ({lxa}|{la}{lb}) K={k} [{lx.lx_kernel_family(lxa, la, lb)}]: max-abs error / sample max = {ratio:.2e}")
+    print(f"config 3 ({lxa}|{la}{lb}) K={k} [{lx.lx_kernel_family_k(lxa, la, lb, k * k)}]: max-abs error / sample max = {ratio:.2e}")
     assert ratio <= CONFIG3_MARGIN[cls], ratio
     qx = oracle.schwarz_aux(cfg["aux"]).max()
     qp = oracle.schwarz_pair(cfg["prim"], cfg["pair_idx"][::16]).max()
