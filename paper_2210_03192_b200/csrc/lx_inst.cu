@@ -45,7 +45,7 @@ static cudaError_t class_launch(const SetMap &map, const DevShells &aux, const D
             return cudaErrorNotSupported;
     } else {
     // Lx = 5, 6 at La+Lb <= 4: one owner warp per ket component (lx_owner.cuh) where the team kernel does not apply
-    constexpr bool has_owner = owner_fits(LX, LA, LB) && (LX >= 5 || !has_team);
+    constexpr bool has_owner = owner_fits(LX, LA, LB) && (LX >= 5 || owner_over_team(LX, LA, LB) || !has_team);
 #ifdef LX_TUNING
     // tuning builds compile every family for every class; LX_FAMILY picks one at run time where it exists
     const int ov = family_override();

@@ -22,13 +22,20 @@
 
 namespace lx {
 
-// does the class (La >= Lb) have an owner kernel?  Lx = 5, 6: La+Lb = 2..4.  Lx = 3, 4: the classes of the chain kernel
-// (La+Lb = 3, 4 where the team kernel does not apply), for weakly contracted launches only (owner_kmax).
+// does the class (La >= Lb) have an owner kernel?  Lx = 5, 6: La+Lb = 2..4.  Lx = 2..4: the classes of the chain kernel (La+Lb =
+// 3, 4 where the team kernel does not apply) and the two team classes where it measured faster, (3|21) and (4|11) — all of them
+// for weakly contracted launches only (owner_kmax).
+__host__ __device__ constexpr bool owner_over_team(int LX, int LA, int LB) {
+    return (LX == 3 && LA == 2 && LB == 1) || (LX == 4 && LA == 1 && LB == 1);
+}
 __host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
-    return LX >= 3 && LX <= LX_MAX_L_AUX && (LA + LB >= (LX >= 5 ? 2 : 3)) && LA + LB <= 4 && LB <= 2 && LA >= LB;
+    if (!(LX <= LX_MAX_L_AUX && LA + LB <= 4 && LB <= 2 && LA >= LB)) return false;
+    if (LX >= 5) return LA + LB >= 2;
+    return (LX >= 2 && LA + LB >= 3) || owner_over_team(LX, LA, LB);
 }
 // largest contraction degree K_a K_b K_x (as known on the host, SetMap.khint) for which the owner kernel is chosen; measured on
-// config 5 (K = 1..4: (3|31) 41 -> 17 ms, (4|31) 43 -> 20 ms, (3|22) 26 -> 14 ms against the chain kernel) and config 2 (K = 9:
+// config 5 (K = 1..4: (3|31) 41 -> 17 ms, (4|31) 43 -> 20 ms, (3|22) 26 -> 14 ms, (2|31) 70 -> 36 ms against the chain kernel,
+// (3|21) 99 -> 73 ms against the team kernel; the other team classes lose) and config 2 (K = 9:
 // the chain / team kernels win for Lx <= 4, the owner kernel for Lx = 5, 6)
 __host__ __device__ constexpr int owner_kmax(int LX, int LA, int LB) {
     return LX >= 5 ? (LA + LB >= 3 ? (1 << 30) : 4) : 4;
@@ -544,9 +551,10 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
     }
 }
 
-// The resident form serves every launch whose K bound fits its buffers, except K = 1 launches of the Lx = 5, 6 classes, where
-// the look-ahead form above (start vectors of the next batch made during the current one) measured faster (LX_OWNER2=0|1 in the
-// environment forces one form: tuning aid).
+// The resident form serves every launch except K = 1 launches of the Lx = 5, 6 classes, where the look-ahead form above (start
+// vectors of the next batch made during the current one) measured 3 % faster ((6|22): 1.64 against 1.69 ms); for contracted
+// launches it wins throughout ((5|22) K = 25: 19.6 against 22.5 ms, (6|22) K = 9: 7.5 against 8.1 ms).  LX_OWNER2=0|1 in the
+// environment forces one form (tuning aid).
 template <int LX, int LA, int LB, int MODE>
 cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                          const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
@@ -557,7 +565,7 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
     long long blocks = (map.nsets + 31) / 32;
     if (blocks > (long long)num_sms) blocks = num_sms;
     static const int force = []() { const char *e = std::getenv("LX_OWNER2"); return e ? (e[0] == '1' ? 1 : 0) : -1; }();
-    bool resident = map.khint > 0 && map.khint <= O2::NSLOT && (LX <= 4 || map.khint > 1);
+    bool resident = !(LX >= 5 && map.khint == 1);
     if (force >= 0) resident = force == 1;
     if (resident) {
         static_assert(O2::smem <= 227 * 1024, "owner kernel (resident form): does not fit in shared memory");
@@ -596,7 +604,7 @@ __host__ __device__ constexpr int team_width(int LX, int LA, int LB) {
 }
 // khint: host-side bound of K_a K_b K_x of the launch, <= 0 = unknown (SetMap.khint)
 __host__ __device__ constexpr int class_family(int LX, int LA, int LB, int khint) {
-    if (owner_fits(LX, LA, LB) && (LX >= 5 || team_width(LX, LA, LB) == 0) &&
+    if (owner_fits(LX, LA, LB) && (LX >= 5 || owner_over_team(LX, LA, LB) || team_width(LX, LA, LB) == 0) &&
         (owner_kmax(LX, LA, LB) == (1 << 30) || (khint > 0 && khint <= owner_kmax(LX, LA, LB))))
         return FAM_OWNER;
     if (team_width(LX, LA, LB) > 0) return FAM_TEAM;
