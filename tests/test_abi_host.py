@@ -54,6 +54,16 @@ def test_workspace_bytes_and_family(lx):
             for lb in range(5):
                 assert lx.lx_kernel_family(lxa, la, lb) in ("team", "chain", "owner", "lane", "group", "slab")
                 assert lx.lx_kernel_family(lxa, la, lb) == lx.lx_kernel_family(lxa, lb, la)
+                for k in (0, 1, 4, 9, 100):
+                    assert lx.lx_kernel_family_k(lxa, la, lb, k) in ("team", "chain", "owner", "lane", "group", "slab")
+                assert lx.lx_kernel_family_k(lxa, la, lb, 0) == lx.lx_kernel_family(lxa, la, lb)
+    # K-aware dispatch: config 2 (K = 9) keeps the round-1 kernels, weakly contracted launches of the chain
+    # classes and every launch of the Lx = 5, 6 classes with La+Lb >= 3 go to the owner kernel, La+Lb = 5, 6 to the slab kernel
+    assert lx.lx_kernel_family_k(4, 2, 2, 9) == "chain" and lx.lx_kernel_family_k(4, 2, 2, 1) == "owner"
+    assert lx.lx_kernel_family_k(2, 1, 1, 1) == "team" and lx.lx_kernel_family_k(3, 2, 1, 2) == "owner"
+    assert lx.lx_kernel_family_k(6, 2, 2, 1) == "owner" and lx.lx_kernel_family_k(5, 2, 2, 25) == "owner"
+    assert lx.lx_kernel_family_k(5, 1, 1, 4) == "owner" and lx.lx_kernel_family_k(5, 1, 1, 9) == "lane"
+    assert lx.lx_kernel_family_k(6, 3, 3, 1) == "slab" and lx.lx_kernel_family_k(4, 4, 4, 1) == "group" and lx.lx_kernel_family_k(1, 3, 2, 1) == "group"
 
 
 def test_shard_pairs_partition():

@@ -108,6 +108,38 @@ def test_every_compiled_class_tiny(lx, oracle, lxa):
             _check(_run(lx, cfg), ref)
 
 
+@pytest.mark.parametrize("cls", [(6, 2, 2), (5, 3, 1), (4, 2, 2), (3, 2, 1), (2, 3, 1), (6, 1, 1), (4, 3, 3), (6, 3, 2), (3, 2, 3)])
+@pytest.mark.parametrize("kprim", [(1, 2), (1, 7), (3, 6)])
+def test_mixed_contraction_batches(lx, oracle, cls, kprim):
+    """Shell pairs of very different contraction degree in one call (K_a, K_b drawn per shell from kprim, aux K 1..2), 70
+    pairs x 9 aux shells = several 32-set batches with different K each: the owner kernel's resident form takes several
+    batches per round and falls back to chunks of primitives where a batch has more primitives than buffers (K up to 72
+    here), the slab kernel runs its contracted passes; the K stride passed is the call's maximum (and once a loose bound)."""
+    lxa, la, lb = cls
+    rng = np.random.default_rng(7000 + 100 * lxa + 10 * la + lb + kprim[1])
+    npair = 70
+    shells = []
+    for i in range(2 * npair):
+        l = la if i < npair else lb
+        k = int(rng.integers(kprim[0], kprim[1] + 1))
+        z = np.exp(rng.uniform(np.log(0.15), np.log(4.0), k))
+        shells.append((l, rng.uniform(0, 5, 3), z, rng.uniform(0.3, 1.0, k) * gen.prim_norm(z, l)))
+    prim = table(shells)
+    xs = []
+    for _ in range(9):
+        k = int(rng.integers(1, 3))
+        z = np.exp(rng.uniform(np.log(0.2), np.log(3.0), k))
+        xs.append((lxa, rng.uniform(0, 5, 3), z, rng.uniform(0.3, 1.0, k) * gen.prim_norm(z, lxa)))
+    aux = table(xs)
+    pairs = np.stack([np.arange(npair), npair + np.arange(npair)], axis=1).astype(np.int32)
+    ref = oracle.eri3_batch(lxa, la, lb, aux, prim, np.arange(9, dtype=np.int32), pairs)
+    kmax = int((prim.K[pairs[:, 0]] * prim.K[pairs[:, 1]]).max())
+    da, dp = lx.DeviceShells(aux), lx.DeviceShells(prim)
+    for kk in (kmax, kmax + 5):
+        got = lx.lx_eri3_batch(lxa, la, lb, da, dp, np.arange(9, dtype=np.int32), pairs, kmax=kk)
+        _check(got.cpu().numpy(), ref)
+
+
 def test_degenerate_geometry(lx, oracle):
     """A = B, P = C (T = 0), all centres equal, same shell twice in a pair (reading G15)."""
     z = np.zeros(3)
