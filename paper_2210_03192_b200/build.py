@@ -48,13 +48,18 @@ def _stale(target, deps):
 def build(verbose=False, force=False, jobs=None):
     os.makedirs(OBJ, exist_ok=True)
     hdrs = _headers()
+    # objects made with other flags (a tuning build with LX_EXTRA_NVCC) must not be reused: the flags are stamped
+    stamp = os.path.join(OBJ, "flags.txt")
+    flags_now = " ".join(NVCC_FLAGS)
+    if not os.path.exists(stamp) or open(stamp).read() != flags_now:
+        force = True
     todo = []
     objs = []
     for obj, src, defs in _units():
         o = os.path.join(OBJ, obj)
         s = os.path.join(CSRC, src)
         objs.append(o)
-        if force or EXTRA or _stale(o, [s] + hdrs):
+        if force or _stale(o, [s] + hdrs):
             todo.append(["nvcc"] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
 
     def run(cmd):
@@ -68,6 +73,8 @@ def build(verbose=False, force=False, jobs=None):
             for log in ex.map(run, todo):
                 if verbose and log:
                     sys.stderr.write(log)
+    with open(stamp, "w") as f:
+        f.write(flags_now)
     if todo or _stale(LIB, objs):
         run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     return LIB

@@ -22,6 +22,9 @@
 
 namespace lx {
 
+#ifndef LX_OWNER_MAXE
+#define LX_OWNER_MAXE 5
+#endif
 // does the class (La >= Lb) have an owner kernel?  Lx = 5, 6: La+Lb = 2..4.  Lx = 2..4: the classes of the chain kernel (La+Lb =
 // 3, 4 where the team kernel does not apply) and the two team classes where it measured faster, (3|21) and (4|11) — all of them
 // for weakly contracted launches only (owner_kmax).
@@ -29,7 +32,8 @@ __host__ __device__ constexpr bool owner_over_team(int LX, int LA, int LB) {
     return (LX == 3 && LA == 2 && LB == 1) || (LX == 4 && LA == 1 && LB == 1);
 }
 __host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
-    if (!(LX <= LX_MAX_L_AUX && LA + LB <= 4 && LB <= 2 && LA >= LB)) return false;
+    if (!(LX <= LX_MAX_L_AUX && LA + LB <= LX_OWNER_MAXE && LB <= 2 && LA >= LB)) return false;
+    if (LA + LB == 5) return true;
     if (LX >= 5) return LA + LB >= 2;
     return (LX >= 2 && LA + LB >= 3) || owner_over_team(LX, LA, LB);
 }
@@ -38,7 +42,7 @@ __host__ __device__ constexpr bool owner_fits(int LX, int LA, int LB) {
 // (3|21) 99 -> 73 ms against the team kernel; the other team classes lose) and config 2 (K = 9:
 // the chain / team kernels win for Lx <= 4, the owner kernel for Lx = 5, 6)
 __host__ __device__ constexpr int owner_kmax(int LX, int LA, int LB) {
-    return LX >= 5 ? (LA + LB >= 3 ? (1 << 30) : 4) : 4;
+    return LX >= 5 || LA + LB >= 5 ? (LA + LB >= 3 ? (1 << 30) : 4) : 4;
 }
 
 template <int LX, int LA, int LB>
@@ -47,7 +51,7 @@ struct OwnCls {
     static constexpr int NXC = nc(LX), NA = nc(LA), NB = nc(LB), NAB = NA * NB, NINT = NXC * NAB;
     static constexpr int NLEV = LX / 2 + 1;                       // levels p = 0..Lx/2, one producer warp each
     // warps per block from the register budget of a consumer (chain copy NG + accumulator NACC doubles, plus scalars)
-    static constexpr int NW = E <= 2 ? 24 : (E == 3 ? 16 : 12);
+    static constexpr int NW = E <= 2 ? 24 : (E == 3 ? 16 : (E == 4 ? 12 : 8));
     // contracted batches (K > 1): warps [0, NWC) own one ket component per pass, warps [NWC, NW) produce
     static constexpr int NWC = NW - NLEV;
     static constexpr int NPASS = (NXC + NWC - 1) / NWC;
@@ -131,7 +135,7 @@ __device__ __forceinline__ void owner_chain(const double *__restrict__ zb, int l
 // once per partner ((6|22): 381 instead of 684 FP64 instructions for c = x⁶).  Each start vector is still read once per partner.
 template <int LX, int LA, int LB, int A>
 __device__ __forceinline__ void owner_partners_axis(int cA, int cB, int cC, const double *__restrict__ ub, int lane,
-                                                    double (&acc)[OwnCls<LX, LA, LB>::NACC]) {
+                                                    double (&acc)[OwnCls<LX, LA, LB>::NACC], double scale) {
     using OC = OwnCls<LX, LA, LB>;
     constexpr int NG = OC::NG, NACC = OC::NACC, NLEV = OC::NLEV;
     constexpr int B = (A + 1) % 3, C = (A + 2) % 3;
@@ -140,7 +144,7 @@ __device__ __forceinline__ void owner_partners_axis(int cA, int cB, int cC, cons
     // integers in double (no integer division in the loop)
     auto grow = [](int ci, int ni) { return (double)((ci - 2 * ni) * (ci - 2 * ni - 1)) * (ni == 0 ? 0.5 : (ni == 1 ? 0.25 : 1.0 / 6.0)); };
     const int NA_ = cA >> 1;
-    double bB = 1.0;
+    double bB = scale;
 #pragma unroll 1
     for (int nB = 0; 2 * nB <= cB; ++nB) {
         double bBC = bB;
@@ -180,20 +184,20 @@ __device__ __forceinline__ void owner_partners_axis(int cA, int cB, int cC, cons
 // 19.6 -> 20.2 ms), where the plain form — one independent chain per partner — overlaps better; each path takes its own.
 template <int LX, int LA, int LB, bool HORNER>
 __device__ __forceinline__ void owner_partners(int c, const double *__restrict__ ub, int lane,
-                                               double (&acc)[OwnCls<LX, LA, LB>::NACC]) {
+                                               double (&acc)[OwnCls<LX, LA, LB>::NACC], double scale = 1.0) {
     using OC = OwnCls<LX, LA, LB>;
     constexpr int E = OC::E, NG = OC::NG, NLEV = OC::NLEV;
     int s = 0;
     while ((s + 1) * (s + 2) / 2 <= c) ++s;                     // s = c_y + c_z
     const int cz = c - s * (s + 1) / 2, cy = s - cz, cx = LX - s;
     if constexpr (HORNER) {
-        if (cx >= cy && cx >= cz) owner_partners_axis<LX, LA, LB, 0>(cx, cy, cz, ub, lane, acc);
-        else if (cy >= cz) owner_partners_axis<LX, LA, LB, 1>(cy, cz, cx, ub, lane, acc);
-        else owner_partners_axis<LX, LA, LB, 2>(cz, cx, cy, ub, lane, acc);
+        if (cx >= cy && cx >= cz) owner_partners_axis<LX, LA, LB, 0>(cx, cy, cz, ub, lane, acc, scale);
+        else if (cy >= cz) owner_partners_axis<LX, LA, LB, 1>(cy, cz, cx, ub, lane, acc, scale);
+        else owner_partners_axis<LX, LA, LB, 2>(cz, cx, cy, ub, lane, acc, scale);
     } else {
         const double rx = ub[(NLEV * NG + 0) * 32 + lane], ry = ub[(NLEV * NG + 1) * 32 + lane], rz = ub[(NLEV * NG + 2) * 32 + lane];
         auto grow = [](int ci, int ni) { return (double)((ci - 2 * ni) * (ci - 2 * ni - 1)) * (ni == 0 ? 0.5 : (ni == 1 ? 0.25 : 1.0 / 6.0)); };
-        double bx = 1.0;
+        double bx = scale;
 #pragma unroll 1
         for (int nx = 0; 2 * nx <= cx; ++nx) {
             double bxy = bx;
@@ -424,11 +428,15 @@ template <int LX, int LA, int LB, int MODE>
 struct Own2Cls {
     using OC = OwnCls<LX, LA, LB>;
     static constexpr int UB = OC::UREC * 32;                              // doubles per start-vector buffer
-    static constexpr int STW = MODE == 1 ? 0 : 32 * OC::SP;               // staging (MODE 0) / J partial sums (MODE 2) per warp
-    static constexpr int fixed = OC::NW * STW * 8 + OWN2_MAXB * (int)sizeof(OwnHdr) + (int)sizeof(Own2Ctl) + 64;
+    static constexpr int SPG = OC::NACC | 1;                              // MODE 2: stride of a set's Σ_c d_c (e0|c)
+    // per warp: staging slot (MODE 0); MODE 2: partial sums, then J rows — written after the round's chains are done, so the
+    // slots ALIAS the start-vector buffers and cost no shared memory (more batches per round)
+    static constexpr int STW = MODE == 1 ? 0 : 32 * OC::SP;
+    static constexpr int fixed = (MODE == 0 ? OC::NW * STW * 8 : 0) + OWN2_MAXB * (int)sizeof(OwnHdr) + (int)sizeof(Own2Ctl) + 64;
     static constexpr int NSLOT = cmin(16, (222 * 1024 - fixed) / (UB * 8));
     static constexpr size_t smem = (size_t)fixed + (size_t)NSLOT * UB * 8;
     static_assert(NSLOT >= 1, "owner kernel: no room for a start-vector buffer");
+    static_assert(MODE != 2 || (size_t)NSLOT * UB >= (size_t)OC::NW * STW, "owner kernel: J slots do not fit the aliased buffers");
 };
 
 template <int LX, int LA, int LB, int MODE>
@@ -443,8 +451,8 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
 
     extern __shared__ double smem[];
     double *U = smem;                                            // [NSLOT][UREC][32]
-    double *ST = U + (size_t)NSLOT * UB;                         // [NW][STW]
-    OwnHdr *hdr = reinterpret_cast<OwnHdr *>(ST + (size_t)NW * STW);
+    double *ST = MODE == 2 ? U : U + (size_t)NSLOT * UB;         // [NW][STW] (MODE 2: aliases U)
+    OwnHdr *hdr = reinterpret_cast<OwnHdr *>(U + (size_t)NSLOT * UB + (MODE == 0 ? (size_t)NW * STW : 0));
     Own2Ctl *ctl = reinterpret_cast<Own2Ctl *>(hdr + OWN2_MAXB);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -474,32 +482,60 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
         const int km = __reduce_max_sync(FULL, K);
         if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; h->next_p = 0; }
     };
-    // a10 for the batch of header h: sum the partial J sums of the warps w = w0, w0 + dw, .. then the lanes that share a pair
+    // a10 (MODE 2).  An owner folds d_c into the weights of its chains and keeps ONE accumulator over all the ket components it
+    // takes: G = Σ_c d_c (e0|c) — the HRR is linear and does not depend on c, so it runs once per batch, not once per component
+    // (the step before the HRR is where the paper's J-engine contracts as well).  The warps w = w0, w0 + dw, ..
+    // worked on the batch of header h: the first of them sums their partial G and transfers it (eq. 1, lane = set) into its
+    // slot; then its lanes take the elements (a, b) and walk the sets: one atomic per run of equal pairs and element (mirrored).
     auto j_reduce = [&](const OwnHdr *h, int w0, int dw) {
-        const int pl_own = h->p[lane];
-        const bool live = pl_own >= 0;
-        const unsigned livemask = __ballot_sync(FULL, live);
-        const int sa = h->a[lane], sb = h->b[lane];
-        for (int r = warp; r < NAB; r += NW) {
-            double v = 0.0;
-            for (int w = w0; w < NW; w += dw) v += ST[(size_t)w * STW + (size_t)lane * SP + r];
-            const int ia = r / NB, ib = r - ia * NB;
-            unsigned rest = livemask;
-            while (rest) {
-                const int leader = __ffs(rest) - 1;
-                const int pl = __shfl_sync(FULL, pl_own, leader);
-                const unsigned grp = __ballot_sync(FULL, live && pl_own == pl) & rest;
-                double sum = (grp >> lane) & 1u ? v : 0.0;
+        constexpr int SPG = O2::SPG;
+        if (warp != w0) return;                                  // one warp per batch: the tail of a round is short
+        double H0[NACC];
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
-                if (lane == leader) {
+        for (int i = 0; i < NACC; ++i) H0[i] = 0.0;
+        for (int w = w0; w < NW; w += dw) {
+            const double *g = ST + (size_t)w * STW + (size_t)lane * SPG;
+            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] += g[decltype(ii)::value]; });
+        }
+        const double AB[3] = {h->AB[0][lane], h->AB[1][lane], h->AB[2][lane]};
+        __syncwarp();
+        hrr_store<LA, LB>(H0, AB, stw + (size_t)lane * SP, false);    // J contributions of the lane's set into the warp's own slot
+        __syncwarp();
+        // lanes over the elements (a, b); the sets of a batch are walked in order, runs of equal pairs are summed and flushed
+        for (int r = lane; r < NAB; r += 32) {
+            const int ia = r / NB, ib = r - ia * NB;
+            int cur = -1, s0 = 0;
+            double sum = 0.0;
+            auto flush = [&]() {
+                if (cur >= 0) {
+                    const int sa = h->a[s0], sb = h->b[s0];
                     const size_t ra0 = prim.bf_off[sa], rb0 = prim.bf_off[sb];
                     atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
                     if (sa != sb) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
                 }
-                rest &= ~grp;
+            };
+#pragma unroll 1
+            for (int ss = 0; ss < 32; ++ss) {
+                const int ps = h->p[ss];
+                if (ps < 0) continue;
+                if (ps != cur) {
+                    flush();
+                    cur = ps;
+                    s0 = ss;
+                    sum = 0.0;
+                }
+                sum += stw[(size_t)ss * SP + r];
             }
+            flush();
         }
+    };
+    // this warp's G (back from the u = f / a! basis) into its slot
+    auto g_store = [&](const double (&acc)[NACC]) {
+        constexpr int SPG = O2::SPG;
+        static_for<0, NACC>([&](auto ii) {
+            constexpr int i = decltype(ii)::value;
+            stw[(size_t)lane * SPG + i] = acc[i] * (double)cart_fact(off(LA) + i);
+        });
     };
 
     long long base = blockIdx.x;
@@ -524,7 +560,6 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
         }
         __syncthreads();
         const int nb = ctl->nb;
-        bool first = true;                                       // MODE 2: this warp's partial J sums are still empty
         if (nb > 0) {
             // ---- start vectors: work items (slot = (batch, primitive), level) ---------------------------------------------------
             const int nitem = ctl->tot * NLEV;
@@ -545,41 +580,51 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
             const int kq = hd->kmax;
             const double *ub0 = U + (size_t)ctl->slot0[ib_] * UB;
             const long long batch = base + ib_ * G;
+            double acc[NACC];
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+            const bool dlive = MODE == 2 && hd->p[lane] >= 0;
+            const double *dvec = MODE == 2 ? df.D + aux.bf_off[hd->x[lane]] : nullptr;
             while (true) {
                 int c = 0;
                 if (lane == 0) c = atomicAdd(&hd->next_c, 1);
                 c = __shfl_sync(FULL, c, 0);
                 if (c >= NXC) break;
-                double acc[NACC];
-#pragma unroll
-                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+                double scale = 1.0;
+                if constexpr (MODE == 2) scale = dlive ? __ldg(dvec + c) : 0.0;
                 if (kq == 1) {
-                    owner_partners<LX, LA, LB, true>(c, ub0, lane, acc);
+                    owner_partners<LX, LA, LB, true>(c, ub0, lane, acc, scale);
                 } else {
 #pragma unroll 1
-                    for (int q = 0; q < kq; ++q) owner_partners<LX, LA, LB, false>(c, ub0 + (size_t)q * UB, lane, acc);
+                    for (int q = 0; q < kq; ++q) owner_partners<LX, LA, LB, false>(c, ub0 + (size_t)q * UB, lane, acc, scale);
                 }
-                owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
-                first = false;
+                if constexpr (MODE != 2) {
+                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, false);
+#pragma unroll
+                    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+                }
             }
             if constexpr (MODE == 2) {
-                if (first) {
-                    for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
-                }
+                __syncthreads();                                 // every warp is done with the start vectors: their space takes the sums
+                g_store(acc);
                 __syncthreads();
-                for (int i = 0; i < nb; ++i) j_reduce(hdr + i, i, nb);
+                j_reduce(hd, ib_, nb);
             }
             base += (long long)nb * G;
         } else {
             // ---- one batch with more primitives than buffers: chunks of NSLOT primitives, one ket component per warp and pass ------
             OwnHdr *hd = hdr;
             const int kmax = hd->kmax;
+            double acc[NACC];
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+            const bool dlive = MODE == 2 && hd->p[lane] >= 0;
+            const double *dvec = MODE == 2 ? df.D + aux.bf_off[hd->x[lane]] : nullptr;
 #pragma unroll 1
             for (int c0 = 0; c0 < NXC; c0 += NW) {
                 const int c = c0 + warp;
-                double acc[NACC];
-#pragma unroll
-                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+                double scale = 1.0;
+                if constexpr (MODE == 2) scale = (dlive && c < NXC) ? __ldg(dvec + c) : 0.0;
 #pragma unroll 1
                 for (int q0 = 0; q0 < kmax; q0 += NSLOT) {
                     const int nq = min(NSLOT, kmax - q0);
@@ -592,18 +637,18 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
                     __syncthreads();
                     if (c < NXC) {
 #pragma unroll 1
-                        for (int q = 0; q < nq; ++q) owner_partners<LX, LA, LB, false>(c, U + (size_t)q * UB, lane, acc);
+                        for (int q = 0; q < nq; ++q) owner_partners<LX, LA, LB, false>(c, U + (size_t)q * UB, lane, acc, scale);
                     }
                 }
-                if (c < NXC) {
-                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df, first);
-                    first = false;
+                if constexpr (MODE != 2) {
+                    if (c < NXC) owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df, false);
+#pragma unroll
+                    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
                 }
             }
             if constexpr (MODE == 2) {
-                if (first) {
-                    for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
-                }
+                __syncthreads();
+                g_store(acc);
                 __syncthreads();
                 j_reduce(hd, 0, 1);
             }
@@ -626,8 +671,10 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
     long long blocks = (map.nsets + 31) / 32;
     if (blocks > (long long)num_sms) blocks = num_sms;
     static const int force = []() { const char *e = std::getenv("LX_OWNER2"); return e ? (e[0] == '1' ? 1 : 0) : -1; }();
+    constexpr bool v1_fits = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr) <= 227 * 1024;
     bool resident = !(LX >= 5 && map.khint == 1);
     if (force >= 0) resident = force == 1;
+    if (!v1_fits || MODE == 2) resident = true;                  // the J digestion of the resident form sums over c in registers
     if (resident) {
         static_assert(O2::smem <= 227 * 1024, "owner kernel (resident form): does not fit in shared memory");
         auto kern = owner2_kernel<LX, LA, LB, MODE>;
@@ -637,12 +684,15 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
         return cudaGetLastError();
     }
     constexpr size_t smem = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr);
-    static_assert(smem <= 227 * 1024, "owner kernel: batch does not fit in shared memory");
-    auto kern = owner_kernel<LX, LA, LB, MODE>;
-    static std::atomic<unsigned long long> configured{0};
-    if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
-    kern<<<(unsigned)blocks, OC::NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
-    return cudaGetLastError();
+    if constexpr (smem <= 227 * 1024) {
+        auto kern = owner_kernel<LX, LA, LB, MODE>;
+        static std::atomic<unsigned long long> configured{0};
+        if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
+        kern<<<(unsigned)blocks, OC::NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+        return cudaGetLastError();
+    } else {
+        return cudaErrorNotSupported;   // not reached: `resident` is always true for these classes
+    }
 }
 
 // ---- kernel family of a class (La >= Lb), shared by the dispatcher (lx_inst.cu) and lx_kernel_family() ------------------

@@ -63,7 +63,8 @@ def test_workspace_bytes_and_family(lx):
     assert lx.lx_kernel_family_k(2, 1, 1, 1) == "team" and lx.lx_kernel_family_k(3, 2, 1, 2) == "owner"
     assert lx.lx_kernel_family_k(6, 2, 2, 1) == "owner" and lx.lx_kernel_family_k(5, 2, 2, 25) == "owner"
     assert lx.lx_kernel_family_k(5, 1, 1, 4) == "owner" and lx.lx_kernel_family_k(5, 1, 1, 9) == "lane"
-    assert lx.lx_kernel_family_k(6, 3, 3, 1) == "slab" and lx.lx_kernel_family_k(4, 4, 4, 1) == "group" and lx.lx_kernel_family_k(1, 3, 2, 1) == "group"
+    assert lx.lx_kernel_family_k(6, 3, 3, 1) == "slab" and lx.lx_kernel_family_k(4, 4, 4, 1) == "group" and lx.lx_kernel_family_k(1, 3, 2, 1) == "owner"
+    assert lx.lx_kernel_family_k(4, 3, 2, 9) == "owner" and lx.lx_kernel_family_k(0, 3, 3, 1) == "group"
 
 
 def test_shard_pairs_partition():
