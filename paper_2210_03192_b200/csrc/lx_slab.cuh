@@ -1,22 +1,23 @@
-// lx_slab.cuh — "slab kernel": the owner scheme of lx_owner.cuh for bra shells too large for one lane (La+Lb >= 5).
+// lx_slab.cuh — "slab kernel": the owner scheme of lx_owner.cuh for La+Lb = 6, where a lane can hold the start vector (84
+// doubles) but not the accumulator next to it, and where the HRR (Lb = 3, or 64 inputs for (x|42)) no longer fits registers.
 //
-// LANE = shell-set as in the team / chain / owner kernels, but the vector over the bra components a (all shells
-// 0..E, E = La+Lb: 56 / 84 / 120 / 165 doubles for E = 5..8) no longer fits a lane's registers.  It is cut into SLABS
-// along x: slab s holds the components with a_x = s, a triangle of the in-slab powers (a_y, a_z), a_y + a_z <= E − s.
-// Everything runs on one slab at a time in registers; what couples the slabs goes through shared memory, where the
-// start vectors live anyway:
+// LANE = shell-set, one owner warp per ket component c as in lx_owner.cuh.  The bra components (all shells 0..E, E = La+Lb)
+// are kept in SLAB-MAJOR order: slab s holds the components with a_x = s, a triangle of the in-slab powers (a_y, a_z),
+// a_y + a_z <= E − s.
 //   a3  VRR1 (eq. 3) as three nested ONE-dimensional pyramids — raising one axis needs no other axis:
 //       the x line [s00]^(m), from row s the y line [s a_y 0]^(m), from each of its rows the z line [s a_y a_z]^(m) — so a
 //       work item (level p, slab s) is independent of every other item and needs no shared memory but for its result;
-//   a4  a chain (lx_chain.cuh) Π B_i^{t_i} on slab s: the x steps by their closed form
-//       (B_x^{t} u)[s] = Σ_j C(t,j) r_x^{t−j} u[s−j]   (loads of the slabs s−j, j <= min(t, s)),
-//       the y and z steps in place in registers (they stay inside a slab); partners and primitives accumulate in registers
-//       (a5), one owner warp per ket component c as in lx_owner.cuh;
-//   a7  the HRR (eq. 1) in the same form: the x part of b by its closed form
-//       Σ_k C(b_x,k) AB_x^{b_x−k} (e0|c)[s+k] (loads), the y and z parts as up-shifting steps in registers;
-//   a8  the finished rows of a shell-set leave through a small staging slot as coalesced runs.
-// All loops over ket components, partners and steps are run-time loops around compile-time slab bodies: the code is a few
-// tens of KB and stays in the instruction cache (lx_owner.cuh explains why that matters for K = 1 classes).
+//   a4  the chains Π B_i^{t_i} (lx_chain.cuh) run on the whole vector in the owner's registers, one read of the start vector
+//       per partner; the sum over partners and primitives (a5) is kept in the owner's (e0|c) region in shared memory;
+//   a7  the HRR (eq. 1) one slab of rows a_x = S at a time: the x part of b by its closed form
+//       Σ_k C(b_x,k) AB_x^{b_x−k} (e0|c)[s+k] (loads of the slabs S..S+b_x), the y and z parts as up-shifting steps in registers;
+//   a8  the finished rows of a shell-set leave through a small staging slot as coalesced runs (a9: contracted with D there;
+//       a10: d_c is contracted BEFORE the HRR, which then runs once per batch).
+// All loops over ket components, partners and steps are run-time loops around compile-time bodies: the code stays in the
+// instruction cache (lx_owner.cuh explains why that matters for K = 1 classes).
+// A first version cut the chains into slabs as well (x steps by the closed form (B_x^t u)[s] = Σ_j C(t,j) r_x^{t−j} u[s−j] from
+// shared memory, teams of two warps per component): 15.3 ms for (6|33) against 14.4 ms now, 10.1 against 7.7 ms for (5|33);
+// La+Lb = 5 moved to the owner kernel altogether (8 warps of 255 registers: 3–5× faster than either slab form).
 #pragma once
 #include "lx_owner.cuh"
 
@@ -26,7 +27,7 @@ namespace lx {
 #define LX_SLAB_MINW32 4
 #endif
 #ifndef LX_SLAB_TEAM
-#define LX_SLAB_TEAM 2
+#define LX_SLAB_TEAM 1
 #endif
 __host__ __device__ constexpr int tsz(int n) { return n * (n + 1) / 2; }                 // components of a triangle of size n
 // slab-major component order of the bra vector (shells 0..E): slab s = a_x, inside by d = a_y + a_z, then a_z
@@ -143,64 +144,47 @@ __device__ __noinline__ void slab_produce(int p, const PrimRec &R, const double 
     });
 }
 
-// In-slab chain steps on the triangle z[d(d+1)/2 + q] (d = a_y + a_z, q = a_z), in place, descending d.
-template <int N, int AXIS, int ZO, int NZ>   // AXIS 1: y (a_y − 1: same q, d − 1), AXIS 2: z (a_z − 1: q − 1, d − 1); triangle at z[ZO..]
-__device__ __forceinline__ void slab_step(double (&z)[NZ], double r) {
-    static_for<0, N>([&](auto id) {
-        constexpr int d = N - 1 - decltype(id)::value;
-        static_for<0, d + 1>([&](auto iq) {
-            constexpr int q = decltype(iq)::value, i = ZO + tsz(d) + q;
-            constexpr bool has = AXIS == 1 ? (d - q > 0) : (q > 0);
-            if constexpr (has) z[i] = fma(r, z[i], z[ZO + tsz(d - 1) + (AXIS == 1 ? q : q - 1)]);
-            else z[i] = r * z[i];
+// ---- chains on the WHOLE bra vector in registers (La+Lb = 6: 84 doubles, 168 registers) -----------------------------------
+// Where one lane can hold the whole start vector — it cannot hold the accumulator as well — the chains run as in the owner
+// kernel (lx_owner.cuh: every step in registers, one read of the start vector per partner, no closed-form x part with its
+// repeated loads) and only the sum over the partners goes through shared memory, into the owner's slab-major (e0|c) region.
+// Measured (B200, config 3): (6|33) 15.3 -> see DESIGN.md section 10.
+template <int E, int AXIS>
+__device__ __forceinline__ void whole_step(double (&z)[off(E + 1)], double r) {
+    // descending total degree t = s + d: the source a − 1_axis (degree t − 1) is still un-stepped when a is
+    static_for<0, E + 1>([&](auto it) {
+        constexpr int t = E - decltype(it)::value;
+        static_for<0, t + 1>([&](auto is) {
+            constexpr int sx = decltype(is)::value, d = t - sx;           // slab sx, in-slab degree d
+            static_for<0, d + 1>([&](auto iq) {
+                constexpr int q = decltype(iq)::value, i = slab_off(E, sx) + tsz(d) + q;
+                constexpr bool has = AXIS == 0 ? sx > 0 : (AXIS == 1 ? d - q > 0 : q > 0);
+                if constexpr (has) {
+                    constexpr int lo = AXIS == 0 ? slab_off(E, sx - 1) + tsz(d) + q
+                                                 : slab_off(E, sx) + tsz(d - 1) + (AXIS == 1 ? q : q - 1);
+                    z[i] = fma(r, z[i], z[lo]);
+                } else {
+                    z[i] = r * z[i];
+                }
+            });
         });
     });
 }
 
-// Slabs are worked on in GROUPS of consecutive slabs whose triangles together stay within a register budget: one run of the
-// partner loops serves a whole group (the small slabs near a_x = E would otherwise pay the loop overhead for a few FMAs).
-#ifndef LX_SLAB_GROUP
-#define LX_SLAB_GROUP 30
-#endif
-struct SlabGroups { int n; int s0[LX_MAX_L_PRIM * 2 + 2]; };      // group g = slabs s0[g] .. s0[g+1]−1
-__host__ __device__ constexpr SlabGroups slab_groups(int E) {
-    SlabGroups g{};
-    g.n = 0;
-    int s = 0;
-    while (s <= E) {
-        g.s0[g.n++] = s;
-        int tot = tsz(E - s + 1);
-        ++s;
-        while (s <= E && tot + tsz(E - s + 1) <= LX_SLAB_GROUP) { tot += tsz(E - s + 1); ++s; }
-    }
-    g.s0[g.n] = E + 1;
-    return g;
-}
-
-// a4/a5 for (ket component c, slab group G): all partners n <= c/2 of the kprim primitives in `ub` (buffers of UREC*NS
-// doubles), accumulated in registers; then scale · (e0|c) = scale · acc · a! of the group's slabs goes to (add: is added to) the
-// owner's E0 region (scale = 1, or d_c when the team sums Σ_c d_c (e0|c) for the J digestion).
-template <int LX, int LA, int LB, int G>
-__device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *__restrict__ ub, int kprim,
-                                         double *__restrict__ e0w, int ls, bool add, double scale) {
+template <int LX, int LA, int LB>
+__device__ __noinline__ void slab_chains_whole(int cx, int cy, int cz, const double *__restrict__ ub, int kprim,
+                                               double *__restrict__ e0w, int ls, bool add, double scale) {
     using SC = SlabCls<LX, LA, LB>;
     constexpr int E = SC::E, NG = SC::NG, NS = SC::NS;
-    constexpr SlabGroups GR = slab_groups(E);
-    constexpr int SA = GR.s0[G], SB = GR.s0[G + 1];                // slabs SA .. SB−1
-    constexpr int ZB = slab_off(E, SA), NZ = slab_off(E, SB) - ZB;  // the group's components are contiguous in slab-major order
-    constexpr int AB0 = e0_off(E, LA, SA), NACCG = e0_off(E, LA, SB) - AB0;
-    double acc[NACCG];
-#pragma unroll
-    for (int i = 0; i < NACCG; ++i) acc[i] = 0.0;
     auto grow = [](int ci, int ni) { return (double)((ci - 2 * ni) * (ci - 2 * ni - 1)) * (ni == 0 ? 0.5 : (ni == 1 ? 0.25 : 1.0 / 6.0)); };
+    bool fresh = !add;                                           // the first partner stores, the others add
 #pragma unroll 1
     for (int q = 0; q < kprim; ++q) {
         const double *uq = ub + (size_t)q * SC::UREC * NS + ls;
-        const double ry = uq[SC::O_RY * NS], rz = uq[SC::O_RZ * NS];
-        double bx = 1.0;
+        const double rx = uq[(size_t)(SC::O_RXP + 1) * NS], ry = uq[SC::O_RY * NS], rz = uq[SC::O_RZ * NS];
+        double bx = scale;
 #pragma unroll 1
         for (int nx = 0; 2 * nx <= cx; ++nx) {
-            const int tx = cx - 2 * nx;
             double bxy = bx;
 #pragma unroll 1
             for (int ny = 0; 2 * ny <= cy; ++ny) {
@@ -209,38 +193,31 @@ __device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *_
                 for (int nz = 0; 2 * nz <= cz; ++nz) {
                     const int p = nx + ny + nz;
                     const double *up = uq + (size_t)p * NG * NS;
-                    // x part: z[S] = Σ_j C(tx,j) r_x^{tx−j} u[S−j] for the slabs S of the group
-                    double z[NZ];
-                    double bj = 1.0;
-                    static_for<0, cmin(LX, SB - 1) + 1>([&](auto ij) {
-                        constexpr int j = decltype(ij)::value;
-                        if (j <= tx) {
-                            const double w = bj * uq[(size_t)(SC::O_RXP + tx - j) * NS];
-                            static_for<cmax(SA, j), SB>([&](auto is) {
-                                constexpr int S = decltype(is)::value, NT = tsz(E - S + 1), zo = slab_off(E, S) - ZB;
-                                const double *us = up + (size_t)slab_off(E, S - j) * NS;
-                                static_for<0, NT>([&](auto ii) {
-                                    constexpr int i = decltype(ii)::value;
-                                    if constexpr (j == 0) z[zo + i] = w * us[(size_t)i * NS];
-                                    else z[zo + i] = fma(w, us[(size_t)i * NS], z[zo + i]);
-                                });
-                            });
-                            bj *= (double)(tx - j) * (1.0 / (double)(j + 1));
-                        }
-                    });
-                    const int ty = cy - 2 * ny, tz = cz - 2 * nz;
+                    double z[NG];
+                    static_for<0, NG>([&](auto ig) { z[decltype(ig)::value] = up[(size_t)decltype(ig)::value * NS]; });
 #pragma unroll 1
-                    for (int k = 0; k < ty; ++k)
-                        static_for<SA, SB>([&](auto is) { slab_step<E - decltype(is)::value + 1, 1, slab_off(E, decltype(is)::value) - ZB, NZ>(z, ry); });
+                    for (int k = cx - 2 * nx; k > 0; --k) whole_step<E, 0>(z, rx);
 #pragma unroll 1
-                    for (int k = 0; k < tz; ++k)
-                        static_for<SA, SB>([&](auto is) { slab_step<E - decltype(is)::value + 1, 2, slab_off(E, decltype(is)::value) - ZB, NZ>(z, rz); });
+                    for (int k = cy - 2 * ny; k > 0; --k) whole_step<E, 1>(z, ry);
+#pragma unroll 1
+                    for (int k = cz - 2 * nz; k > 0; --k) whole_step<E, 2>(z, rz);
                     const double ck = beta * uq[(size_t)(SC::O_CK + p) * NS];
-                    static_for<SA, SB>([&](auto is) {
-                        constexpr int S = decltype(is)::value, n = E - S + 1, T0 = tsz(slab_dmin(LA, S));
-                        constexpr int zo = slab_off(E, S) - ZB, ao = e0_off(E, LA, S) - AB0;
-                        static_for<0, tsz(n) - T0>([&](auto ii) { acc[ao + decltype(ii)::value] = fma(ck, z[zo + T0 + decltype(ii)::value], acc[ao + decltype(ii)::value]); });
+                    // acc (shared memory, slab-major, shells >= LA, back in the f = u a! basis) += ck z
+                    static_for<0, E + 1>([&](auto is) {
+                        constexpr int sx = decltype(is)::value, n = E - sx + 1, DMIN = slab_dmin(LA, sx), T0 = tsz(DMIN);
+                        double *dst = e0w + (size_t)(e0_off(E, LA, sx) - T0) * NS + ls;
+                        static_for<DMIN, n>([&](auto id) {
+                            constexpr int d = decltype(id)::value;
+                            static_for<0, d + 1>([&](auto iq) {
+                                constexpr int qq = decltype(iq)::value, i = tsz(d) + qq;
+                                constexpr double f = (double)ifact(sx) * (double)ifact(d - qq) * (double)ifact(qq);
+                                const double v = (ck * f) * z[slab_off(E, sx) + i];
+                                if (fresh) dst[(size_t)i * NS] = v;
+                                else dst[(size_t)i * NS] += v;
+                            });
+                        });
                     });
+                    fresh = false;
                     beta *= grow(cz, nz);
                 }
                 bxy *= grow(cy, ny);
@@ -248,21 +225,6 @@ __device__ __noinline__ void slab_chains(int cx, int cy, int cz, const double *_
             bx *= grow(cx, nx);
         }
     }
-    // back from the u = f / a! basis; slab-major (e0|c) region of the owner
-    double *dst = e0w + (size_t)AB0 * NS + ls;
-    static_for<SA, SB>([&](auto is) {
-        constexpr int S = decltype(is)::value, n = E - S + 1, DMIN = slab_dmin(LA, S), T0 = tsz(DMIN);
-        constexpr int ao = e0_off(E, LA, S) - AB0;
-        static_for<DMIN, n>([&](auto id) {
-            constexpr int d = decltype(id)::value;
-            static_for<0, d + 1>([&](auto iq) {
-                constexpr int q = decltype(iq)::value, i = ao + tsz(d) + q - T0;
-                constexpr double f = (double)ifact(S) * (double)ifact(d - q) * (double)ifact(q);
-                if (add) dst[(size_t)i * NS] = fma(acc[i], f * scale, dst[(size_t)i * NS]);
-                else dst[(size_t)i * NS] = acc[i] * (f * scale);
-            });
-        });
-    });
 }
 
 // a7 + a8 for the rows a with a_x = S of one ket component: (a b| = Σ_{k <= b} Π_i C(b_i,k_i) AB_i^{b_i−k_i} (a+k 0| (eq. 1
@@ -453,14 +415,10 @@ __host__ __device__ constexpr int snake(int k, int T) { return (k % (2 * T)) < T
 template <int LX, int LA, int LB>
 __device__ __forceinline__ void slab_component_chains(int c, int wt, const double *__restrict__ ub, int kprim,
                                                       double *__restrict__ e0t, int ls, bool add, double scale) {
-    constexpr int E = LA + LB, T = SlabCls<LX, LA, LB>::T;
     int s = 0;
     while ((s + 1) * (s + 2) / 2 <= c) ++s;
     const int cz = c - s * (s + 1) / 2, cy = s - cz, cx = LX - s;
-    static_for<0, slab_groups(E).n>([&](auto ig) {
-        constexpr int g = decltype(ig)::value;
-        if (wt == snake(g, T)) slab_chains<LX, LA, LB, g>(cx, cy, cz, ub, kprim, e0t, ls, add, scale);
-    });
+    if (wt == 0) slab_chains_whole<LX, LA, LB>(cx, cy, cz, ub, kprim, e0t, ls, add, scale);
 }
 // the rows (a_x = S) team member wt transfers and stores (MODE 0) or contracts with D into γ (MODE 1, a9: PAPER.md:283, :365)
 template <int LX, int LA, int LB, int MODE>
