@@ -144,7 +144,12 @@ size_t lx_df_workspace_bytes(const lx_schedule_t *s);
  * lx_df_J — row a10.
  *   J[(bf(a)+ca)*ldJ + bf(b)+cb] = Σ_{X,cx} (X_cx|a_ca b_cb) d[bf(X)+cx], mirrored to (b,a); J (nbf×nbf) is
  *   overwritten in full (blocks of unlisted or fully screened pairs become zero).
- * aux / prim: the same tables the schedule was built from, with DEVICE array members (bf_off required). */
+ * aux / prim: the same tables the schedule was built from, with DEVICE array members (bf_off required).
+ * Stream semantics: the class launches of a pass are independent, so where they are small (fewer than 2 M shell-sets per
+ * launch on average) the library spreads them over a few internal side
+ * streams (environment LX_DF_STREAMS, read by lx_init, default 4 including `stream`; 1 = `stream` only) that are forked from
+ * `stream` after the pre-pass and joined to it before the call returns: work queued on `stream` after the call sees the finished
+ * result, as with a single stream.  The two DF calls are not re-entrant (one call at a time per process). */
 int lx_df_gamma(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *D, int ldD,
                 double *gamma, void *workspace, size_t workspace_bytes, void *stream);
 int lx_df_J(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *d, double *J,

@@ -33,6 +33,13 @@ struct State {
     // asynchronous status word in device memory, OR-ed into by the kernels (lx_async_status)
     int *flag_dev = nullptr;
     int check = 0;                   // LX_CHECK=1 in the environment (read by lx_init)
+    // side streams of the DF drivers: the class launches of a pass are independent (they only add into gamma / J), so their
+    // tails overlap when they are spread over a few streams (LX_DF_STREAMS, default 4; 1 = the caller's stream only)
+    static constexpr int MAX_SIDE = 7;
+    int n_side = 0;
+    cudaStream_t side[MAX_SIDE] = {};
+    cudaEvent_t side_ev[MAX_SIDE] = {};
+    cudaEvent_t fork_ev = nullptr;
 };
 static State g;
 static std::mutex g_mu;
@@ -313,6 +320,13 @@ static void free_device_state() {
     if (g.boys_tab) cudaFree(g.boys_tab);
     if (g.arena) cudaFree(g.arena);
     if (g.flag_dev) cudaFree(g.flag_dev);
+    for (int i = 0; i < g.n_side; ++i) {
+        cudaStreamDestroy(g.side[i]);
+        cudaEventDestroy(g.side_ev[i]);
+    }
+    if (g.fork_ev) cudaEventDestroy(g.fork_ev);
+    g.n_side = 0;
+    g.fork_ev = nullptr;
     for (int l = 0; l <= LX_MAX_L_AUX; ++l) {
         if (g.solid[l]) cudaFree(g.solid[l]);
         g.solid[l] = nullptr;
@@ -338,6 +352,17 @@ int lx_init(int device) {
     }
     LX_CUDA(cudaMalloc((void **)&g.flag_dev, sizeof(int)));
     LX_CUDA(cudaMemset(g.flag_dev, 0, sizeof(int)));
+    {
+        const char *e = std::getenv("LX_DF_STREAMS");
+        int n = e ? std::atoi(e) : 4;
+        n = std::max(1, std::min(n, State::MAX_SIDE + 1)) - 1;
+        LX_CUDA(cudaEventCreateWithFlags(&g.fork_ev, cudaEventDisableTiming));
+        for (int i = 0; i < n; ++i) {
+            LX_CUDA(cudaStreamCreateWithFlags(&g.side[i], cudaStreamNonBlocking));
+            LX_CUDA(cudaEventCreateWithFlags(&g.side_ev[i], cudaEventDisableTiming));
+            g.n_side = i + 1;
+        }
+    }
     cudaDeviceProp prop;
     LX_CUDA(cudaGetDeviceProperties(&prop, device));
     g.num_sms = prop.multiProcessorCount;
@@ -734,14 +759,31 @@ static int df_run(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shell
     int rc;
     for (const auto &pb : s->pair_b)
         if ((rc = launch_pair_data(dprim, pb.d_pairs, (int)pb.q.size(), 0, pb.d_pd_off, pb.kmax, pd, st)) != LX_OK) return rc;
+    // fork: the side streams wait for the pre-pass (and for the caller's memset of the output); the launches go round the
+    // streams; join: the caller's stream waits for every side stream.  Stream order is all the synchronisation the pass needs.
+    // Only where the launches are small: measured (B200) config 4 (280 k sets per launch) 11.9 -> 10.4 ms with four streams, config 5
+    // (10 M sets per launch) 2.23 -> 2.43 s — large launches fill the GPU by themselves and only disturb each other.
+    const bool small_launches = !s->launches.empty() && s->nsets / (long long)s->launches.size() < 2000000LL;
+    const int ns = small_launches ? g.n_side : 0;
+    if (ns > 0) {
+        LX_CUDA(cudaEventRecord(g.fork_ev, st));
+        for (int i = 0; i < ns; ++i) LX_CUDA(cudaStreamWaitEvent(g.side[i], g.fork_ev, 0));
+    }
+    int turn = 0;
     for (const auto &l : s->launches) {
         const auto &ab = s->aux_b[l.ab];
         const auto &pb = s->pair_b[l.pb];
         SetMap map{l.nsets, (int)ab.ids.size(), (int)pb.q.size(), ab.d_ids, pb.d_pairs, l.d_cum, pb.kmax * ab.K};
         PairData pdat{pd, pb.d_pd_off, pb.kmax};
-        cudaError_t e = k_launch[mode][ab.L](pb.la, pb.lb, map, daux, dprim, pdat, g.boys_tab, nullptr, 0, df, g.num_sms, st);
+        cudaStream_t ls = turn == 0 ? st : g.side[turn - 1];
+        turn = (turn + 1) % (ns + 1);
+        cudaError_t e = k_launch[mode][ab.L](pb.la, pb.lb, map, daux, dprim, pdat, g.boys_tab, nullptr, 0, df, g.num_sms, ls);
         g.launches++;
         if (e != cudaSuccess) return cuda_fail(e);
+    }
+    for (int i = 0; i < ns; ++i) {
+        LX_CUDA(cudaEventRecord(g.side_ev[i], g.side[i]));
+        LX_CUDA(cudaStreamWaitEvent(st, g.side_ev[i], 0));
     }
     return LX_OK;
 }
