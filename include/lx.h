@@ -42,6 +42,7 @@ extern "C" {
 #define LX_ENOMEM (-3)        /* workspace too small (see the *_workspace_bytes functions)                      */
 #define LX_ECUDA (-4)         /* CUDA runtime error; text via lx_strerror(LX_ECUDA)                             */
 #define LX_ENOTINIT (-5)      /* lx_init() has not been called on this device                                   */
+#define LX_ELIMIT (-6)        /* problem larger than the fixed scratch of lx_eri3_batch_static                 */
 
 /* Gaussian shell table, structure of arrays (a shell is a centre, exponents ζ, contraction
  * coefficients and l, over unnormalised primitives).  Immutable during a call. */
@@ -154,6 +155,27 @@ int lx_df_gamma(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_
                 double *gamma, void *workspace, size_t workspace_bytes, void *stream);
 int lx_df_J(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *prim, const double *d, double *J,
             int ldJ, void *workspace, size_t workspace_bytes, void *stream);
+
+/* lx_eri3_batch_static — lx_eri3_batch for callers that must not allocate and have no workspace to pass (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation, same kernels, same result and
+ * argument meaning as lx_eri3_batch, but the primitive-pair data (row a1: 48 bytes per primitive pair) lives in a fixed
+ * array in device memory that the library itself holds: LX_STATIC_SCRATCH_BYTES = 4 MiB on EVERY GPU that loads the
+ * library, from the first use of the library on that GPU until the process exits.
+ *   limit:     npair * kmax_pair * 48 bytes <= LX_STATIC_SCRATCH_BYTES (87 381 primitive pairs, e.g. 9 709 shell pairs of
+ *              K_a K_b = 9); beyond it the call returns LX_ELIMIT and launches nothing.  kmax_pair >= max K_a K_b over
+ *              the listed pairs (explicit here; a pair above it comes back as NaN and lx_async_status() says LX_ENOMEM).
+ *   allocates: nothing — no cudaMalloc / cudaFree / allocating library routine; lx_init(device), which must have been
+ *              called, has looked up the array's device address.  The first launch of a class kernel in a process loads
+ *              its code and sets its shared-memory attribute (CUDA lazy loading): run each class once before a capture.
+ *   sharing:   every call uses the SAME array and leaves its contents behind.  Nothing in it has to start at zero: a call
+ *              rewrites every record it reads.  Calls that overlap on the GPU (different streams, or another process
+ *              thread) RACE on it: issue them on one stream, or order them with events.  lx_eri3_batch with caller
+ *              workspaces is the entry point for concurrent calls. */
+#define LX_STATIC_SCRATCH_BYTES (4u << 20)
+size_t lx_static_scratch_bytes(void);
+int lx_eri3_batch_static(int lx, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim,
+                         const int32_t *x_idx, int nx, const int32_t *pair_idx, int npair, int kmax_pair,
+                         double *out, void *stream);
 
 /* Host-buffer convenience path (used for the end-to-end measurement): same result as lx_eri3_batch but every
  * array member of aux/prim, x_idx, pair_idx and out are HOST pointers; the call allocates device scratch, copies

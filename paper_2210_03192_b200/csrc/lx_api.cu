@@ -33,6 +33,7 @@ struct State {
     // asynchronous status word in device memory, OR-ed into by the kernels (lx_async_status)
     int *flag_dev = nullptr;
     int check = 0;                   // LX_CHECK=1 in the environment (read by lx_init)
+    double *static_scratch = nullptr;   // device address of lx_static_scratch on the current device (lx_eri3_batch_static)
     // side streams of the DF drivers: the class launches of a pass are independent (they only add into gamma / J), so their
     // tails overlap when they are spread over a few streams (LX_DF_STREAMS, default 4; 1 = the caller's stream only)
     static constexpr int MAX_SIDE = 7;
@@ -292,6 +293,12 @@ static int launch_pair_data(const DevShells &prim, const int32_t *pair_list, int
 
 using namespace lx;
 
+// Scratch of the allocation-free entry point lx_eri3_batch_static (include/lx.h): the primitive-pair data (row a1) of ONE
+// call.  File scope, fixed size: every GPU that loads the library holds these 4 MiB until the process exits.  In host code
+// the name is only a stand-in for the symbol, not a device address: lx_init() asks cudaGetSymbolAddress for the address on
+// the device it initialises and the entry point hands THAT to the kernels.
+static __device__ __align__(256) double lx_static_scratch[LX_STATIC_SCRATCH_BYTES / sizeof(double)];
+
 // ================================================================================================ C ABI
 extern "C" {
 
@@ -312,6 +319,7 @@ const char *lx_strerror(int status) {
         case LX_ENOMEM: return "workspace too small";
         case LX_ECUDA: return g.cuda_msg;
         case LX_ENOTINIT: return "lx_init() has not been called";
+        case LX_ELIMIT: return "npair * kmax_pair exceeds the fixed scratch of lx_eri3_batch_static (LX_STATIC_SCRATCH_BYTES = 4 MiB = 87381 primitive pairs): use lx_eri3_batch with a workspace";
         default: return "unknown status";
     }
 }
@@ -335,6 +343,7 @@ static void free_device_state() {
     g.arena = nullptr;
     g.arena_bytes = 0;
     g.flag_dev = nullptr;
+    g.static_scratch = nullptr;
     g.ready = false;
 }
 
@@ -352,6 +361,12 @@ int lx_init(int device) {
     }
     LX_CUDA(cudaMalloc((void **)&g.flag_dev, sizeof(int)));
     LX_CUDA(cudaMemset(g.flag_dev, 0, sizeof(int)));
+    {
+        // device address of the static scratch array on THIS device (lx_eri3_batch_static); checked like every other call
+        void *p = nullptr;
+        LX_CUDA(cudaGetSymbolAddress(&p, lx_static_scratch));
+        g.static_scratch = reinterpret_cast<double *>(p);
+    }
     {
         const char *e = std::getenv("LX_DF_STREAMS");
         int n = e ? std::atoi(e) : 4;
@@ -514,6 +529,37 @@ int lx_eri3_batch(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shel
     // khint: the stride bounds K_a K_b; the aux contraction is not known on the host (aux shells are mostly uncontracted)
     SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr, kstride};
     PairData pdat{pd, nullptr, kstride};
+    DfArgs df{nullptr, nullptr, 0};
+    cudaError_t e = k_launch[0][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
+    g.launches++;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return LX_OK;
+}
+
+size_t lx_static_scratch_bytes(void) { return (size_t)LX_STATIC_SCRATCH_BYTES; }
+
+// Allocation-free variant of lx_eri3_batch (include/lx.h): pre-pass and class kernel as there, primitive-pair data in the
+// library's static device array.  No cudaMalloc / cudaFree here or below: launch_pair_data and the class launchers only launch.
+int lx_eri3_batch_static(int lx_, int la, int lb, const lx_shells_t *aux, const lx_shells_t *prim, const int32_t *x_idx,
+                         int nx, const int32_t *pair_idx, int npair, int kmax_pair, double *out, void *stream) {
+    if (!g.ready || !g.static_scratch) return LX_ENOTINIT;
+    if (nx < 0 || npair < 0) return LX_EINVAL;
+    if (!class_supported(lx_, la, lb)) return LX_EUNSUPPORTED;
+    if (nx == 0 || npair == 0) return LX_OK;
+    int rc;
+    if ((rc = check_shells(aux, false)) != LX_OK) return rc;
+    if ((rc = check_shells(prim, false)) != LX_OK) return rc;
+    if (!x_idx || !pair_idx || !out || kmax_pair < 1) return LX_EINVAL;
+    if ((unsigned long long)npair * (unsigned long long)kmax_pair * PD_STRIDE * sizeof(double) > (unsigned long long)LX_STATIC_SCRATCH_BYTES)
+        return LX_ELIMIT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int swapped = la < lb ? 1 : 0;
+    const int cla = swapped ? lb : la, clb = swapped ? la : lb;
+    DevShells dprim = dev_view(prim), daux = dev_view(aux);
+    double *pd = g.static_scratch;           // the looked-up device address, never the symbol's host-side name
+    if ((rc = launch_pair_data(dprim, pair_idx, npair, swapped, nullptr, kmax_pair, pd, st)) != LX_OK) return rc;
+    SetMap map{(long long)npair * nx, nx, npair, x_idx, pair_idx, nullptr, kmax_pair};
+    PairData pdat{pd, nullptr, kmax_pair};
     DfArgs df{nullptr, nullptr, 0};
     cudaError_t e = k_launch[0][lx_](cla, clb, map, daux, dprim, pdat, g.boys_tab, out, swapped, df, g.num_sms, st);
     g.launches++;

@@ -17,14 +17,14 @@ if not os.path.exists(_SO):
                       "there is no CPU fallback")
 _lib = C.CDLL(_SO)
 
-LX_OK, LX_EINVAL, LX_EUNSUPPORTED, LX_ENOMEM, LX_ECUDA, LX_ENOTINIT = 0, -1, -2, -3, -4, -5
+LX_OK, LX_EINVAL, LX_EUNSUPPORTED, LX_ENOMEM, LX_ECUDA, LX_ENOTINIT, LX_ELIMIT = 0, -1, -2, -3, -4, -5, -6
 LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
            "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family", "lx_kernel_family_k",
            "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status",
-           "lx_schwarz_aux_host", "lx_schwarz_pair_host"]
+           "lx_schwarz_aux_host", "lx_schwarz_pair_host", "lx_eri3_batch_static", "lx_static_scratch_bytes"]
 
 
 class lx_shells_t(C.Structure):
@@ -188,6 +188,30 @@ def lx_eri3_batch(lx, la, lb, aux, prim, x_idx, pair_idx, out=None, workspace=No
     _check(_lib.lx_eri3_batch(lx, la, lb, C.byref(aux.struct), C.byref(prim.struct), x_idx.data_ptr(), nx,
                               pair_idx.data_ptr(), npair, out.data_ptr(), workspace.data_ptr(),
                               min(workspace.numel(), need), _stream_ptr(stream)))
+    return out
+
+
+_lib.lx_static_scratch_bytes.restype = C.c_size_t
+_lib.lx_static_scratch_bytes.argtypes = []
+_lib.lx_eri3_batch_static.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(lx_shells_t), C.POINTER(lx_shells_t), C.c_void_p, C.c_int,
+                                      C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+
+
+def lx_static_scratch_bytes():
+    return int(_lib.lx_static_scratch_bytes())
+
+
+def lx_eri3_batch_static(lx, la, lb, aux, prim, x_idx, pair_idx, out, kmax, stream=None):
+    """lx_eri3_batch without a workspace and without any allocation in the library: the primitive-pair data lives in the
+    library's static device array (4 MiB; LxError(LX_ELIMIT) beyond npair * kmax * 48 bytes).  `out`, `x_idx` and `pair_idx`
+    must be device tensors the caller made (this wrapper allocates nothing either)."""
+    assert isinstance(x_idx, torch.Tensor) and isinstance(pair_idx, torch.Tensor) and isinstance(out, torch.Tensor)
+    assert x_idx.dtype == torch.int32 and pair_idx.dtype == torch.int32 and out.dtype == torch.float64
+    assert x_idx.is_cuda and pair_idx.is_cuda and out.is_cuda and x_idx.is_contiguous() and pair_idx.is_contiguous() and out.is_contiguous()
+    nx, npair = x_idx.numel(), pair_idx.numel() // 2
+    assert out.numel() == npair * nx * ncart(lx) * ncart(la) * ncart(lb)
+    _check(_lib.lx_eri3_batch_static(lx, la, lb, C.byref(aux.struct), C.byref(prim.struct), x_idx.data_ptr(), nx,
+                                     pair_idx.data_ptr(), npair, int(kmax), out.data_ptr(), _stream_ptr(stream)))
     return out
 
 
