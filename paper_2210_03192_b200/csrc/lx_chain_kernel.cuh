@@ -47,19 +47,13 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         const long long sid = bb * 32 + lane;
         const bool live = sid < map.nsets;
         int p = 0, xs = 0;
-        if (live) {
-            if (map.cum == nullptr) {
+        if (map.cum == nullptr) {
+            if (live) {
                 p = (int)(sid / map.nx);
                 xs = (int)(sid - (long long)p * map.nx);
-            } else {
-                int lo = 0, hi_ = map.npair;             // largest p with cum[p] <= sid
-                while (hi_ - lo > 1) {
-                    const int mid = (lo + hi_) >> 1;
-                    if (map.cum[mid] <= sid) lo = mid; else hi_ = mid;
-                }
-                p = lo;
-                xs = (int)(sid - map.cum[p]);
             }
+        } else {
+            find_pair_warp(map, sid, live, p, xs);               // the whole warp 0 is here (lane = set)
         }
         const int a = map.pair_list[2 * p + swapped], b = map.pair_list[2 * p + 1 - swapped];
         const int x = map.x_list[xs];

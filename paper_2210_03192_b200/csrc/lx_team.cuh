@@ -157,23 +157,68 @@ __device__ __forceinline__ void chain_apply_reg(const double (&u)[off(E + 1)], c
 
 // ---- shell-set of a lane ------------------------------------------------------------------------------------------
 struct SetId { int p, a, b, x; bool live; };
+
+// Prefix map (DF calls): the pair of a set id is the largest p with cum[p] <= sid.  A per-lane binary search over up to 3.3 M
+// pairs (config 5) is a chain of 22 DEPENDENT global loads at the head of every batch — for weakly contracted classes longer
+// than the arithmetic of the batch (ncu: long-scoreboard stalls 2.5–6 per issue, profiles/r02_ncu_team_df.md).  The 32 set ids
+// of a warp are consecutive, so the warp searches ONCE, 32-ary (5 rounds for 3.3 M pairs: every lane probes one point, a ballot
+// counts the points at or below the first id), then one coalesced load of the next 32 pair starts places every lane.
+// All 32 lanes must call; lane 0 holds the smallest id and every id lies within 32 of it.
+__device__ __forceinline__ void find_pair_warp(const SetMap &map, long long sid, bool live, int &p, int &xs) {
+    constexpr unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const long long sid0 = __shfl_sync(FULL, sid, 0);
+    p = 0;
+    xs = 0;
+    if (sid0 >= map.nsets) return;                            // warp-uniform: no live set
+    int lo = 0, hi = map.npair;                                // cum[lo] <= sid0 < cum[hi]
+    while (hi - lo > 1) {
+        const int step = (hi - lo + 31) >> 5;
+        const long long idx = (long long)lo + (long long)(lane + 1) * step;
+        const bool ok = idx < hi && map.cum[idx] <= sid0;      // cum is non-decreasing: the lanes that say yes are a prefix
+        const int cnt = __popc(__ballot_sync(FULL, ok));
+        lo += cnt * step;
+        hi = min(hi, lo + step);
+    }
+    const int P0 = lo;
+    const long long jn = (long long)P0 + 1 + lane;
+    const long long c = jn <= map.npair ? map.cum[jn] : 0x7fffffffffffffffLL;   // start of pair P0 + 1 + lane
+    long long start = map.cum[P0];
+    int cnt = 0, j = 0;
+#pragma unroll 1
+    for (; j < 32; ++j) {
+        const long long cj = __shfl_sync(FULL, c, j);
+        if (cj > sid0 + 31) break;                             // warp-uniform: no id of this warp reaches pair P0 + 1 + j
+        if (cj <= sid) { ++cnt; start = cj; }
+    }
+    int pp = P0 + cnt;
+    if (cnt == 32 && live) {                                   // more than 32 pairs inside one batch (sparse survivors): finish alone
+        int l2 = P0 + 32, h2 = map.npair;
+        while (h2 - l2 > 1) {
+            const int mid = (l2 + h2) >> 1;
+            if (map.cum[mid] <= sid) l2 = mid; else h2 = mid;
+        }
+        pp = l2;
+        start = map.cum[pp];
+    }
+    if (live) {
+        p = pp;
+        xs = (int)(sid - start);
+    }
+}
+
+// With a prefix map every lane of the warp must call (find_pair_warp).
 __device__ __forceinline__ SetId decode_set(const SetMap &map, long long sid, int swapped) {
     SetId s;
     s.live = sid < map.nsets;
     int p = 0, xs = 0;
-    if (s.live) {
-        if (map.cum == nullptr) {
+    if (map.cum == nullptr) {
+        if (s.live) {
             p = (int)(sid / map.nx);
             xs = (int)(sid - (long long)p * map.nx);
-        } else {
-            int lo = 0, hi = map.npair;                 // largest p with cum[p] <= sid
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (map.cum[mid] <= sid) lo = mid; else hi = mid;
-            }
-            p = lo;
-            xs = (int)(sid - map.cum[p]);
         }
+    } else {
+        find_pair_warp(map, sid, s.live, p, xs);
     }
     s.p = p;
     s.a = map.pair_list[2 * p + swapped];
