@@ -139,7 +139,7 @@ struct ChainCls {
     static constexpr int NW = P.nw;
     static constexpr int NUB = (T.n - NXC) * NACC * 32;       // staging of the contracted targets of the levels p >= 1
     static constexpr int ZBD = cmax(P.ring, NUB);             // the staging area aliases the ring
-    static constexpr int HDR1 = 9 * 32 + 32 + 6 * 16 + 4;     // header: 9 doubles + 1 int64 + 6 ints per set + kmax, in doubles
+    static constexpr int HDR1 = 9 * 32 + 32 + 7 * 16 + 4;     // header: 9 doubles + 1 int64 + 7 ints per set + kmax, in doubles
     static constexpr int HDRD = 2 * HDR1;                     // double-buffered (the next batch is decoded ahead)
     static constexpr size_t smem = ((size_t)32 * SLOTN + (size_t)ZBD + HDRD + 4) * 8 + 2048;   // + partner table
     static constexpr bool fits = E <= 4 && LX <= 4 && P.ok && smem <= 227 * 1024 && NW <= 32;
@@ -151,7 +151,7 @@ __host__ __device__ constexpr bool chain_fits(int LX, int LA, int LB) {
     int NT = 0;
     for (int p = 0; 2 * p <= LX; ++p) NT += nc(LX - 2 * p);
     const int nub = (NT - nc(LX)) * NACC * 32;
-    const size_t smem = ((size_t)32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) + (size_t)cmax(P.ring, nub) + 2 * (9 * 32 + 32 + 6 * 16 + 4) + 4) * 8 + 2048;
+    const size_t smem = ((size_t)32 * ((nc(LX) * nc(LA) * nc(LB)) | 1) + (size_t)cmax(P.ring, nub) + 2 * (9 * 32 + 32 + 7 * 16 + 4) + 4) * 8 + 2048;
     return P.ok && smem <= 227 * 1024 && P.nw <= 32;
 }
 

@@ -43,7 +43,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         double *hd = hd0 + (size_t)hb * CC::HDR1;
         long long *hpo = reinterpret_cast<long long *>(hd + 9 * 32);
         int *hi = reinterpret_cast<int *>(hpo + 32);
-        int *s_kmax = hi + 6 * 32;
+        int *s_kmax = hi + 7 * 32;
         const long long sid = bb * 32 + lane;
         const bool live = sid < map.nsets;
         int p = 0, xs = 0;
@@ -73,6 +73,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         hi[3 * 32 + lane] = a;
         hi[4 * 32 + lane] = b;
         hi[5 * 32 + lane] = x;
+        hi[6 * 32 + lane] = p;
         const int km = __reduce_max_sync(FULL, K);
         if (lane == 0) *s_kmax = km;
     };
@@ -82,7 +83,7 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         const double *hd = hd0 + (size_t)hbuf * CC::HDR1;    // this batch's header (decoded during the previous batch)
         const long long *hpo = reinterpret_cast<const long long *>(hd + 9 * 32);
         const int *hi = reinterpret_cast<const int *>(hpo + 32);
-        const int *s_kmax = hi + 6 * 32;
+        const int *s_kmax = hi + 7 * 32;
         __syncthreads();
         const int kmax = *s_kmax;
         // the finished shell-sets of the previous batch are still in TC (nothing writes TC before the end of the first
@@ -250,7 +251,16 @@ chain_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const dou
         }
         __syncthreads();
         if constexpr (PURE) pure_epilogue<LX, LA, LB, NW, CSTR, SLOTN>(TC, ZB, df.D, warp, lane, batch, map, prim, out, swapped);
-        else chain_epilogue<LX, LA, LB, MODE, NW, true>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+        else {
+            // the lane's shell-set, from the batch header in shared memory (decoded one batch ahead by warp 0)
+            SetId sid;
+            sid.a = hi[3 * 32 + lane];
+            sid.b = hi[4 * 32 + lane];
+            sid.x = hi[5 * 32 + lane];
+            sid.p = hi[6 * 32 + lane];
+            sid.live = batch * 32 + lane < map.nsets;
+            chain_epilogue<LX, LA, LB, MODE, NW, true>(TC, ZB, pt, warp, lane, batch, map, aux, prim, out, swapped, df, sid);
+        }
     }
     // the last batch of this block (the epilogue ended with a block barrier)
     if constexpr (MODE == 0) {

@@ -350,13 +350,14 @@ template <int LX, int LA, int LB, int MODE, int NW, bool DEFER = false>
 __device__ __forceinline__ void chain_epilogue(double *__restrict__ TC, const double *__restrict__ UB,
                                                const PartnerTab *__restrict__ pt, int warp, int lane,
                                                long long batch, const SetMap &map, const DevShells &aux,
-                                               const DevShells &prim, double *__restrict__ out, int swapped, const DfArgs &df) {
+                                               const DevShells &prim, double *__restrict__ out, int swapped, const DfArgs &df,
+                                               const SetId &sid) {
     using CC = ChainCls<LX, LA, LB>;
     constexpr int E = CC::E, NACC = CC::NACC, NXC = CC::NXC, NA = CC::NA, NB = CC::NB, NAB = CC::NAB;
     constexpr int NINT = CC::NINT, SLOTN = CC::SLOTN;
     constexpr unsigned FULL = 0xffffffffu;
-    const SetId sid = decode_set(map, batch * 32 + lane, swapped);
-    // a mirrored class (caller's order [c][b][a]) gets its shell-sets transposed by the HRR stores, not by the copy-out
+    // sid: the lane's shell-set (the caller has decoded it: a second search of the prefix map per batch is a second chain of
+    // dependent global loads).  A mirrored class (caller's order [c][b][a]) gets its shell-sets transposed by the HRR stores, not by the copy-out
     const bool tr = MODE == 0 && swapped != 0;
     if constexpr (LB > 0 || LX >= 2) {
         double AB[3];
@@ -582,7 +583,7 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
         });
         __syncthreads();
         if constexpr (MODE == 3) pure_epilogue<LX, LA, LB, W>(TC, UB, df.D, warp, lane, batch, map, prim, out, swapped);
-        else chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df);
+        else chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df, sid);
     }
 }
 
