@@ -1,20 +1,22 @@
-// lx_owner.cuh — "owner kernel": the chain form of lx_chain.cuh with ONE OWNER PER KET COMPONENT, for high aux angular
-// momentum (Lx = 5, 6) at La+Lb <= 4.
+// lx_owner.cuh — "owner kernel": the chain form of lx_chain.cuh with ONE OWNER PER KET COMPONENT, for weakly contracted
+// launches and for high aux angular momentum (which classes: owner_fits / owner_kmax below).
 //
 // The resummed ket recurrence (lx_chain.cuh header; eq. 2 of the paper, plus the c−1 terms of reading G4)
 //
 //     [a0|c]^(0) = Σ_{n <= c/2}  β(c,n) (2ζc)^{−|n|} (2(γ+ζc))^{−|c−2n|} ( Π_i B_i^{c_i − 2n_i} Y_{|n|} )[a]
 //
-// is evaluated here per ket component c: a consumer warp (LANE = shell-set, 32 sets per batch) owns one c per pass, runs
-// the chains of ALL its partners n on the start vectors Y_p / a! (shared memory, written by the producer warps: one
-// warp per level p = 0..Lx/2) and sums them, weighted by the integers β, into one register accumulator — over the
-// partners and over the primitives (a5, "early contraction").  Compared with the team / chain kernels
-// (one chain per DISTINCT target (p, t), then a gather through shared memory) a level-p chain is run once per c that
-// needs it (119 chains instead of 50 targets for Lx = 6), but nothing is staged: the finished (e0|c) of the 32 sets is
-// in the owner's registers, goes through the HRR (a7, eq. 1) right there and leaves through a private
-// 32 × nc(La)nc(Lb) staging slot as a coalesced run (a8) or is digested (a9/a10).  Shared memory holds only
-// the start vectors (double-buffered over the primitive loop) and the staging slots, so that Lx = 5, 6 fit where the
-// (e0|c) region of the chain kernel (32 sets × nc(Lx) × NACC doubles) does not.
+// is evaluated here per ket component c: a warp (LANE = shell-set, 32 sets per batch) takes a component, runs the chains of
+// ALL its partners n on the start vectors Y_p / a! in shared memory and sums them, weighted by the integers β, into one
+// register accumulator — over the partners and over the primitives (a5, "early contraction").  Compared with
+// the team / chain kernels (one chain per DISTINCT target (p, t), then a gather through shared memory) a level-p chain is run
+// once per c that needs it (119 chains instead of 50 targets for Lx = 6), but nothing is staged: the finished (e0|c) of the 32
+// sets is in the owner's registers, goes through the HRR (a7, eq. 1) right there and leaves through a private
+// 32 × nc(La)nc(Lb) staging slot as a coalesced run (a8) or is digested (a9/a10).  Shared memory holds only the
+// start vectors and the staging slots, so that Lx = 5, 6 fit where the (e0|c) region of the chain kernel (32 sets × nc(Lx) ×
+// NACC doubles) does not, and the per-batch cost (no passes, no gather, no idle epilogue warps) is small enough for K ≈ 1.
+// The kernel ("resident form") is owner2_kernel below.  A first form with dedicated producer warps, a double-buffered primitive
+// loop and the start vectors of the next batch made ahead was slower on contracted launches ((5|22) K = 25: 22.5 against
+// 19.6 ms) and, in the end, on K = 1 launches as well ((6|22): 1.75 against 1.54 ms); it was removed.
 #pragma once
 #include <cstdlib>
 
@@ -49,16 +51,11 @@ template <int LX, int LA, int LB>
 struct OwnCls {
     static constexpr int E = LA + LB, NG = off(E + 1), NACC = NG - off(LA);
     static constexpr int NXC = nc(LX), NA = nc(LA), NB = nc(LB), NAB = NA * NB, NINT = NXC * NAB;
-    static constexpr int NLEV = LX / 2 + 1;                       // levels p = 0..Lx/2, one producer warp each
+    static constexpr int NLEV = LX / 2 + 1;                       // levels p = 0..Lx/2
     // warps per block from the register budget of a consumer (chain copy NG + accumulator NACC doubles, plus scalars)
     static constexpr int NW = E <= 2 ? 24 : (E == 3 ? 16 : (E == 4 ? 12 : 8));
-    // contracted batches (K > 1): warps [0, NWC) own one ket component per pass, warps [NWC, NW) produce
-    static constexpr int NWC = NW - NLEV;
-    static constexpr int NPASS = (NXC + NWC - 1) / NWC;
-    static constexpr int NCP = (NXC + NPASS - 1) / NPASS;         // ket components per pass (balanced over the passes)
     static constexpr int SP = NAB | 1;                            // staging stride of a set (odd: conflict-free both ways)
     static constexpr int UREC = NLEV * NG + 3 + NLEV;             // doubles per set of one start-vector buffer: u, r[3], ck[p]
-    static_assert(NWC >= 1 && NCP <= NWC, "consumer warps cover a pass");
 };
 
 // Batch header in shared memory (lane = set).
@@ -68,12 +65,12 @@ struct OwnHdr {
     int xo0[32], Kab[32], K[32], a[32], b[32], x[32], p[32];
     int tr[32];    // slab kernel: the set is stored transposed ([c][b][a]: mirrored class, or roles exchanged for La = Lb)
     int kmax;      // largest K of the batch (0: no live set)
-    int ready;     // the start vectors of this (K = 1) batch were made ahead, during the previous batch
-    int next_c;    // K = 1 batches: next ket component to hand out (warps take components dynamically)
+    int ready;     // (unused)
+    int next_c;    // next ket component of the batch to hand out (warps take components dynamically)
     int next_p;    // slab kernel: next producer work item
 };
 
-// Producer: start vectors Y_p / a! (a3, eq. 3) of primitive q for the 32 sets of the batch; warp `pw` makes level pw.
+// Start vectors Y_p / a! (a3, eq. 3) of primitive q, level pw, for the 32 sets of the batch (one work item of a warp).
 // Buffer layout [UREC][32]: u[p][g], r[3] = 2γ(P−C), ck[p] = (1/(2(γ+ζc)))^{Lx−2p} (1/(2ζc))^p.
 template <int LX, int LA, int LB>
 __device__ __forceinline__ void owner_produce(double *__restrict__ ub, const OwnHdr *hd, int q, int pw, int lane,
@@ -268,149 +265,6 @@ __device__ __forceinline__ void owner_finish(int c, const double (&acc)[OwnCls<L
             double *js = stw + (size_t)lane * SP;
 #pragma unroll
             for (int i = 0; i < NAB; ++i) js[i] = first ? fin[i] * dc : fma(fin[i], dc, js[i]);
-        }
-    }
-}
-
-template <int LX, int LA, int LB, int MODE>
-__global__ void __launch_bounds__(OwnCls<LX, LA, LB>::NW * 32, 1)
-owner_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const double *__restrict__ boys_tab,
-             double *__restrict__ out, int swapped, DfArgs df) {
-    using OC = OwnCls<LX, LA, LB>;
-    constexpr int NACC = OC::NACC, NXC = OC::NXC, NB = OC::NB, NAB = OC::NAB;
-    constexpr int NLEV = OC::NLEV, NW = OC::NW, NWC = OC::NWC, NPASS = OC::NPASS, NCP = OC::NCP, SP = OC::SP, UREC = OC::UREC;
-    constexpr unsigned FULL = 0xffffffffu;
-
-    extern __shared__ double smem[];
-    double *U = smem;                                            // [2][UREC][32]
-    double *ST = U + (size_t)2 * UREC * 32;                      // [NW][32][SP]: staging (MODE 0) / J partial sums (MODE 2)
-    OwnHdr *hd2 = reinterpret_cast<OwnHdr *>(ST + (size_t)NW * 32 * SP);   // two headers: the next batch is decoded ahead
-
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const long long nbatch = (map.nsets + 31) / 32;
-    const bool tr = MODE == 0 && swapped != 0;                   // mirrored class: the caller's order is [c][b][a]
-    double *stw = ST + (size_t)warp * 32 * SP;
-
-    // header of batch bb (one warp, lane = set); batches past the end decode as empty (kmax = 0)
-    auto decode = [&](long long bb, OwnHdr *h) {
-        const SetId sid = decode_set(map, bb * 32 + lane, swapped);
-        const int Kab = min(prim.K[sid.a] * prim.K[sid.b], pdat.kstride);
-        const int K = sid.live ? Kab * aux.K[sid.x] : 0;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            const double Ad = prim.center[3 * sid.a + d];
-            h->A[d][lane] = Ad;
-            h->C[d][lane] = aux.center[3 * sid.x + d];
-            h->AB[d][lane] = Ad - prim.center[3 * sid.b + d];
-        }
-        h->po[lane] = pdat.pd_off ? pdat.pd_off[sid.p] : (long long)sid.p * pdat.kstride;
-        h->xo0[lane] = aux.prim_off[sid.x];
-        h->Kab[lane] = Kab;
-        h->K[lane] = K;
-        h->a[lane] = sid.a;
-        h->b[lane] = sid.b;
-        h->x[lane] = sid.x;
-        h->p[lane] = sid.live ? sid.p : -1;
-        const int km = __reduce_max_sync(FULL, K);
-        if (lane == 0) { h->kmax = km; h->ready = 0; h->next_c = 0; h->next_p = 0; }
-    };
-    if (warp == NWC) decode(blockIdx.x, hd2);
-
-    int it = 0;
-    for (long long batch = blockIdx.x; batch < nbatch; batch += gridDim.x, ++it) {
-        __syncthreads();                                         // the previous batch is finished; this batch's header is there
-        OwnHdr *hd = hd2 + (it & 1), *hn = hd2 + ((it + 1) & 1);
-        const int kmax = hd->kmax;
-        bool first = true;                                       // MODE 2: this warp's partial J sums are still empty
-
-        if (kmax <= 1) {
-            // ============ K = 1 batch: start vectors once, then every warp takes ket components until none is left ============
-            double *ub = U + (size_t)(it & 1) * UREC * 32;
-            if (!hd->ready) {                                    // not made ahead (first batch of the block, or after a K > 1 batch)
-                if (warp >= NWC) owner_produce<LX, LA, LB>(ub, hd, 0, warp - NWC, lane, aux, pdat, boys_tab);
-                __syncthreads();
-            }
-            if (warp >= NWC) {
-                // look ahead: header of the next batch and, if it is a K = 1 batch too, its start vectors into the idle buffer
-                if (warp == NWC) decode(batch + gridDim.x, hn);
-                named_sync(2, NLEV * 32);
-                if (hn->kmax == 1) {
-                    owner_produce<LX, LA, LB>(U + (size_t)((it + 1) & 1) * UREC * 32, hn, 0, warp - NWC, lane, aux, pdat, boys_tab);
-                    if (warp == NWC && lane == 0) hn->ready = 1;
-                }
-            }
-            while (true) {
-                int c = 0;
-                if (lane == 0) c = atomicAdd(&hd->next_c, 1);
-                c = __shfl_sync(FULL, c, 0);
-                if (c >= NXC) break;
-                double acc[NACC];
-#pragma unroll
-                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
-                owner_partners<LX, LA, LB, true>(c, ub, lane, acc);
-                owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
-                first = false;
-            }
-        } else {
-            // ============ contracted batch: passes over the ket components, the primitive loop inside each pass ===========
-            if (warp == NWC) decode(batch + gridDim.x, hn);
-#pragma unroll 1
-            for (int pass = 0; pass < NPASS; ++pass) {
-                const int c = pass * NCP + warp;
-                const bool has = warp < NCP && c < NXC;
-                if (warp >= NWC) owner_produce<LX, LA, LB>(U, hd, 0, warp - NWC, lane, aux, pdat, boys_tab);
-                named_sync(1, NW * 32);
-                double acc[NACC];
-#pragma unroll
-                for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
-#pragma unroll 1
-                for (int q = 0; q < kmax; ++q) {
-                    if (warp >= NWC) {
-                        if (q + 1 < kmax) owner_produce<LX, LA, LB>(U + (size_t)((q + 1) & 1) * UREC * 32, hd, q + 1, warp - NWC, lane, aux, pdat, boys_tab);
-                    } else if (has) {
-                        owner_partners<LX, LA, LB, false>(c, U + (size_t)(q & 1) * UREC * 32, lane, acc);
-                    }
-                    named_sync(1, NW * 32);                      // primitive q is consumed, q + 1 is produced
-                }
-                if (has) {
-                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, first);
-                    first = false;
-                }
-            }
-        }
-
-        if constexpr (MODE == 2) {
-            // a10: J[bf(a)+ia, bf(b)+ib] += Σ_X Σ_c (c|ab) d[bf(X)+c], mirrored: sum the warps' partial sums, then the lanes
-            // that share a shell pair (contiguous runs of the batch) by shuffles; one atomic per run and element
-            if (first) {
-                for (int i = 0; i < NAB; ++i) stw[(size_t)lane * SP + i] = 0.0;
-            }
-            __syncthreads();
-            const int pl_own = hd->p[lane];
-            const bool live = pl_own >= 0;
-            const unsigned livemask = __ballot_sync(FULL, live);
-            const int sa = hd->a[lane], sb = hd->b[lane];
-            for (int r = warp; r < NAB; r += NW) {
-                double v = 0.0;
-#pragma unroll
-                for (int w = 0; w < NW; ++w) v += ST[((size_t)w * 32 + lane) * SP + r];
-                const int ia = r / NB, ib = r - ia * NB;
-                unsigned rest = livemask;
-                while (rest) {
-                    const int leader = __ffs(rest) - 1;
-                    const int pl = __shfl_sync(FULL, pl_own, leader);
-                    const unsigned grp = __ballot_sync(FULL, live && pl_own == pl) & rest;
-                    double sum = (grp >> lane) & 1u ? v : 0.0;
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
-                    if (lane == leader) {
-                        const size_t ra0 = prim.bf_off[sa], rb0 = prim.bf_off[sb];
-                        atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
-                        if (sa != sb) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
-                    }
-                    rest &= ~grp;
-                }
-            }
         }
     }
 }
@@ -657,10 +511,6 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
     }
 }
 
-// The resident form serves every launch except K = 1 launches of the Lx = 5, 6 classes, where the look-ahead form above (start
-// vectors of the next batch made during the current one) measured 3 % faster ((6|22): 1.64 against 1.69 ms); for contracted
-// launches it wins throughout ((5|22) K = 25: 19.6 against 22.5 ms, (6|22) K = 9: 7.5 against 8.1 ms).  LX_OWNER2=0|1 in the
-// environment forces one form (tuning aid).
 template <int LX, int LA, int LB, int MODE>
 cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShells &prim, const PairData &pdat,
                          const double *boys_tab, double *out, int swapped, const DfArgs &df, int num_sms,
@@ -670,29 +520,12 @@ cudaError_t owner_launch(const SetMap &map, const DevShells &aux, const DevShell
     if (map.nsets <= 0) return cudaSuccess;
     long long blocks = (map.nsets + 31) / 32;
     if (blocks > (long long)num_sms) blocks = num_sms;
-    static const int force = []() { const char *e = std::getenv("LX_OWNER2"); return e ? (e[0] == '1' ? 1 : 0) : -1; }();
-    constexpr bool v1_fits = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr) <= 227 * 1024;
-    bool resident = !(LX >= 5 && map.khint == 1);
-    if (force >= 0) resident = force == 1;
-    if (!v1_fits || MODE == 2) resident = true;                  // the J digestion of the resident form sums over c in registers
-    if (resident) {
-        static_assert(O2::smem <= 227 * 1024, "owner kernel (resident form): does not fit in shared memory");
-        auto kern = owner2_kernel<LX, LA, LB, MODE>;
-        static std::atomic<unsigned long long> configured{0};
-        if (cudaError_t e = ensure_dyn_smem(kern, O2::smem, configured); e != cudaSuccess) return e;
-        kern<<<(unsigned)blocks, OC::NW * 32, O2::smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
-        return cudaGetLastError();
-    }
-    constexpr size_t smem = ((size_t)2 * OC::UREC * 32 + (size_t)OC::NW * 32 * OC::SP) * 8 + 2 * sizeof(OwnHdr);
-    if constexpr (smem <= 227 * 1024) {
-        auto kern = owner_kernel<LX, LA, LB, MODE>;
-        static std::atomic<unsigned long long> configured{0};
-        if (cudaError_t e = ensure_dyn_smem(kern, smem, configured); e != cudaSuccess) return e;
-        kern<<<(unsigned)blocks, OC::NW * 32, smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
-        return cudaGetLastError();
-    } else {
-        return cudaErrorNotSupported;   // not reached: `resident` is always true for these classes
-    }
+    static_assert(O2::smem <= 227 * 1024, "owner kernel: does not fit in shared memory");
+    auto kern = owner2_kernel<LX, LA, LB, MODE>;
+    static std::atomic<unsigned long long> configured{0};
+    if (cudaError_t e = ensure_dyn_smem(kern, O2::smem, configured); e != cudaSuccess) return e;
+    kern<<<(unsigned)blocks, OC::NW * 32, O2::smem, stream>>>(map, aux, prim, pdat, boys_tab, out, swapped, df);
+    return cudaGetLastError();
 }
 
 // ---- kernel family of a class (La >= Lb), shared by the dispatcher (lx_inst.cu) and lx_kernel_family() ------------------
