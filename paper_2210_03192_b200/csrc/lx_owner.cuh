@@ -289,6 +289,9 @@ struct Own2Cls {
     static constexpr int fixed = (MODE == 0 ? OC::NW * STW * 8 : 0) + OWN2_MAXB * (int)sizeof(OwnHdr) + (int)sizeof(Own2Ctl) + 64;
     static constexpr int NSLOT = cmin(16, (222 * 1024 - fixed) / (UB * 8));
     static constexpr size_t smem = (size_t)fixed + (size_t)NSLOT * UB * 8;
+    // A batch with more primitives than buffers runs in chunks; its warps work in lock-step there, so in the store mode the
+    // staging slots (used only after the last chunk of a pass) lend their space to more buffers: fewer chunks, fewer barriers
+    static constexpr int NSLOT_C = MODE == 0 ? cmin(16, (int)(((size_t)NSLOT * UB + (size_t)OC::NW * STW) / UB)) : NSLOT;
     static_assert(NSLOT >= 1, "owner kernel: no room for a start-vector buffer");
     static_assert(MODE != 2 || (size_t)NSLOT * UB >= (size_t)OC::NW * STW, "owner kernel: J slots do not fit the aliased buffers");
 };
@@ -300,7 +303,7 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
     using OC = OwnCls<LX, LA, LB>;
     using O2 = Own2Cls<LX, LA, LB, MODE>;
     constexpr int NACC = OC::NACC, NXC = OC::NXC, NB = OC::NB, NAB = OC::NAB, NLEV = OC::NLEV, NW = OC::NW, SP = OC::SP;
-    constexpr int UB = O2::UB, NSLOT = O2::NSLOT, STW = O2::STW;
+    constexpr int UB = O2::UB, NSLOT = O2::NSLOT, NSLOT_C = O2::NSLOT_C, STW = O2::STW;
     constexpr unsigned FULL = 0xffffffffu;
 
     extern __shared__ double smem[];
@@ -480,9 +483,9 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
                 double scale = 1.0;
                 if constexpr (MODE == 2) scale = (dlive && c < NXC) ? __ldg(dvec + c) : 0.0;
 #pragma unroll 1
-                for (int q0 = 0; q0 < kmax; q0 += NSLOT) {
-                    const int nq = min(NSLOT, kmax - q0);
-                    __syncthreads();                             // the previous chunk is consumed
+                for (int q0 = 0; q0 < kmax; q0 += NSLOT_C) {
+                    const int nq = min(NSLOT_C, kmax - q0);
+                    __syncthreads();                             // the previous chunk is consumed (and the previous pass is stored)
 #pragma unroll 1
                     for (int item = warp; item < nq * NLEV; item += NW) {
                         const int sq = item / NLEV, lev = item - sq * NLEV;
@@ -494,6 +497,7 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
                         for (int q = 0; q < nq; ++q) owner_partners<LX, LA, LB, false>(c, U + (size_t)q * UB, lane, acc, scale);
                     }
                 }
+                if constexpr (MODE == 0 && NSLOT_C > NSLOT) __syncthreads();   // the staging slots overlap the buffers of the last chunk
                 if constexpr (MODE != 2) {
                     if (c < NXC) owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df, false);
 #pragma unroll
