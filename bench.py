@@ -321,6 +321,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-df", action="store_true", help="skip the DF-J (configs 4, 5) and solid-harmonic side measurements")
     ap.add_argument("--no-side", action="store_true", help="skip the config 1 / config 3 side measurements")
+    ap.add_argument("--df-once", default="", choices=["", "4", "5"],
+                    help="profiling aid: ONE lx_df_gamma + ONE lx_df_J call on configs[3] (4) or configs[4] (5) with GPU-made Schwarz "
+                         "factors, print the two times and exit")
     ap.add_argument("--c3", default="", help="profiling aid: run ONLY the given config-3 class, e.g. '6,3,3,1' (lx,la,lb,kprim), "
                                              "three calls at full size (4096 pairs x 128 aux shells), print its time and exit")
     args = ap.parse_args()
@@ -346,6 +349,21 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     lx.lx_init(local)
 
+    if args.df_once:
+        cfg = gen.config4() if args.df_once == "4" else gen.config5()
+        ha, hp = lx.HostShells(cfg["aux"]), lx.HostShells(cfg["prim"])
+        qx, qp = lx.lx_schwarz_aux_host(ha), lx.lx_schwarz_pair_host(hp, cfg["pair_idx"])
+        sched = lx.Schedule(ha, hp, qx, qp, cfg["pair_idx"], cfg["tau"])
+        da, dp = lx.DeviceShells(ha, dev), lx.DeviceShells(hp, dev)
+        D, d = torch.from_numpy(cfg["D"]).to(dev), torch.from_numpy(cfg["d"]).to(dev)
+        ws = torch.empty(sched.workspace_bytes, dtype=torch.uint8, device=dev)
+        gam = torch.empty(cfg["aux"].nbf, dtype=torch.float64, device=dev)
+        J = torch.empty((cfg["prim"].nbf, cfg["prim"].nbf), dtype=torch.float64, device=dev)
+        mg = _time_calls(lambda: lx.lx_df_gamma(sched, da, dp, D, gamma=gam, workspace=ws), 1)[0]
+        mj = _time_calls(lambda: lx.lx_df_J(sched, da, dp, d, J=J, workspace=ws), 1)[0]
+        print(json.dumps({"df_once": args.df_once, "shell_sets": sched.num_sets, "gamma_ms": mg, "J_ms": mj,
+                          "check_gamma_dot_d": float(gam @ d), "check_J_dot_D": float((J * D).sum())}))
+        return
     if args.c3:
         lxa, la, lb, k = (int(v) for v in args.c3.split(","))
         cfg = gen.config3(lxa, la, lb, kprim=k)
