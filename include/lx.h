@@ -219,8 +219,8 @@ size_t lx_eri3_pure_workspace_bytes(int lx, int la, int lb, int nx, int npair, i
 int lx_solid_matrix(int l, double *matrix_host);
 
 /* Which kernel template serves a class: "team" (register-only chain form, lx_team.cuh), "chain" (warp-specialised
- * chain form, lx_chain_kernel.cuh), "owner" (one owner warp per ket component, lx_owner.cuh), "slab" (the same with the bra
- * vector cut into slabs, lx_slab.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
+ * chain form, lx_chain_kernel.cuh), "owner" (one owner warp per ket component, lx_owner.cuh), "slab" (the same for La+Lb = 6
+ * with slab-wise VRR1 and HRR, lx_slab.cuh), "lane" (bra component per lane, lx_lane.cuh) or "group" (shared-memory,
  * lx_group.cuh); "" if the class is outside the compiled range.  Static storage.  For reports only.
  * Some classes have two families and choose by the contraction degree of the launch ("K-aware
  * dispatch"): lx_kernel_family_k takes the bound K_a K_b K_x the caller knows for the launch (what lx_eri3_batch derives from
