@@ -33,7 +33,8 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/cl
 HBM_PEAK_GBS = 6555.5                                   # BASELINE.md §2 (MEASURED_PEAKS.json of round 1; overridden below if the file is there)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the tracked ncu --set full summaries under
 # profiles/ (never measured by this run: ncu is not available inside a timed bench); class -> (bytes, source file)
-NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): (1.072485e9 + 1.226e6, "profiles/r02_ncu_chain_4_2_2.md (ncu --set full capture, round 2)")}
+NCU_422_WRITE, NCU_422_READ = 1.072212e9, 1.057e6
+NCU_DRAM_BYTES_PER_LAUNCH = {(4, 2, 2): (NCU_422_WRITE + NCU_422_READ, "profiles/r02_ncu_chain_4_2_2.md (ncu --set full capture, end of round 2)")}
 # SURVEY.md §8(d) table, flops per shell-set for the classes it lists (K = 9 for config 2; config 3 as stated there)
 SURVEY_FLOPS_PER_SET = {(0, 0, 0): 414, (1, 1, 1): 2286, (2, 1, 1): 6156, (2, 2, 2): 24816, (3, 2, 2): 52970,
                         (4, 1, 1): 29322, (4, 2, 2): 111054}
@@ -288,6 +289,28 @@ def bench_df(lx, dev, costmodel, cfg, name, reps, unscreened=False):
         return mg, mj
     mg, mj = run(sched)
     lhs, rhs = float(gam @ d), float((J * D).sum())
+    # end to end for the digestion path: D and d come from pinned host memory, gamma and J go back to pinned host memory, all
+    # inside the timed interval (wall clock around copies + both passes + synchronisation); tables and schedule are resident
+    D_h, d_h = torch.from_numpy(cfg["D"]).pin_memory(), torch.from_numpy(cfg["d"]).pin_memory()
+    g_h = torch.empty(aux.nbf, dtype=torch.float64).pin_memory()
+    J_h = torch.empty((prim.nbf, prim.nbf), dtype=torch.float64).pin_memory()
+
+    def e2e_once():
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        D.copy_(D_h, non_blocking=True)
+        d.copy_(d_h, non_blocking=True)
+        lx.lx_df_gamma(sched, da, dp, D, gamma=gam, workspace=ws)
+        lx.lx_df_J(sched, da, dp, d, J=J, workspace=ws)
+        g_h.copy_(gam, non_blocking=True)
+        J_h.copy_(J, non_blocking=True)
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * 1e3
+    e2e_once()
+    e2e_ms = min(e2e_once() for _ in range(max(1, reps)))
+    e2e = {"df_j_ms": e2e_ms, "integrals_per_s": 2 * sched.num_integrals / (e2e_ms * 1e-3),
+           "h2d_bytes": int(D_h.numel() * 8 + d_h.numel() * 8), "d2h_bytes": int(g_h.numel() * 8 + J_h.numel() * 8),
+           "note": "wall clock: H2D of D and d from pinned memory, lx_df_gamma, lx_df_J, D2H of gamma and J, synchronise"}
     fl = _df_model_flops(costmodel, aux, prim, pairs, qx, qp, tau)
     floor_ms = fl / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
     res = {"workload": name, "screening": f"Schwarz, tau = {tau:g}, factors made on the GPU (lx_schwarz_aux_host / lx_schwarz_pair_host)",
@@ -298,7 +321,7 @@ def bench_df(lx, dev, costmodel, cfg, name, reps, unscreened=False):
            "integrals_per_s": 2 * sched.num_integrals / ((mg + mj) * 1e-3),
            "fp64_floor_ms_per_pass_costmodel": floor_ms, "frac_of_fp64_floor": 2 * floor_ms / (mg + mj),
            "check_gamma_dot_d": lhs, "check_J_dot_D": rhs, "check_rel_diff": abs(lhs - rhs) / max(abs(lhs), 1e-300),
-           "schwarz_s": t_q, "schedule_s": t_s}
+           "schwarz_s": t_q, "schedule_s": t_s, "e2e": e2e}
     if unscreened:
         s0 = lx.Schedule(ha, hp, None, None, pairs, 0.0)
         ug, uj = run(s0)
@@ -515,11 +538,13 @@ def main():
         i_top = int(np.argmax(class_ms))
         c_top = classes[i_top]
         canon = (c_top[0], max(c_top[1:]), min(c_top[1:]))
-        # algorithmic flops per shell-set: the component-level DAG count of costmodel.py; SURVEY.md
-        # §8(d) quotes a larger figure for some classes (it over-counts: ncu's executed DFMA/DMUL/DADD count of the
-        # full-OS lane kernel matches the cost model, profiles/r01_ncu_lane_4_2_2.md) and is reported next to it
-        fl_set = costmodel.flops_per_set(*c_top, 9)
+        # algorithmic flops per shell-set: SURVEY.md section 8(d)'s per-unit figure where it lists the class (the primary count,
+        # as the round-1 review asked), the component-level DAG count of costmodel.py beside it (it lowers along the axis with
+        # the smallest positive power: fewer four-term nodes); ncu's executed count is in
+        # profiles/r02_flops_per_class.md
+        fl_model = costmodel.flops_per_set(*c_top, 9)
         fl_survey = SURVEY_FLOPS_PER_SET.get(canon)
+        fl_set = fl_survey if fl_survey else fl_model
         t_top = class_ms[i_top] * 1e-3
         achieved = fl_set * nsets / t_top / 1e12
         roofline = {"bound": "alu", "kernel": f"{lx.lx_kernel_family_k(*canon, 9)}_kernel<{canon[0]},{canon[1]},{canon[2]},0> class ({c_top[0]}|{c_top[1]}{c_top[2]})",
@@ -528,8 +553,9 @@ def main():
                     "traffic_source": NCU_DRAM_BYTES_PER_LAUNCH.get(canon, (None, "no ncu capture of this class under profiles/"))[1],
                     "peak_kind": "nominal FP64 DFMA pipe (148 SM x 64 FMA/clk x 1.965 GHz), DESIGN.md",
                     "peak_measured_dfma_probe": probe, "flops_per_set": fl_set,
-                    "flops_per_set_survey": fl_survey,
-                    "frac_with_survey_flops": (fl_survey * nsets / t_top / 1e12 / FP64_NOMINAL_TFLOPS) if fl_survey else None,
+                    "flops_source": "SURVEY.md section 8(d)" if fl_survey else "costmodel.py (class not in SURVEY.md section 8(d)'s table)",
+                    "flops_per_set_costmodel": fl_model,
+                    "frac_with_costmodel_flops": fl_model * nsets / t_top / 1e12 / FP64_NOMINAL_TFLOPS,
                     "kernel_ms": class_ms[i_top],
                     "share_of_step": float(class_ms[i_top] / class_ms.sum()),
                     "hbm_write_gbs": nint_set(c_top) * 8 * nsets / t_top / 1e9}
