@@ -160,3 +160,41 @@ def test_df_config5_sampled(lx, oracle):
     assert eg <= TOL_DF and eJ <= TOL_DF, (eg, eJ)
     lhs, rhs = float(gamma @ c5["d"]), float(np.sum(J * c5["D"]))
     assert abs(lhs - rhs) <= 1e-10 * np.linalg.norm(gamma) * np.linalg.norm(c5["d"]), (lhs, rhs)
+
+
+@pytest.mark.parametrize("cls", [(2, 1, 1), (3, 2, 1), (4, 3, 1), (5, 3, 2), (6, 3, 3), (0, 0, 0)])
+def test_df_ragged_prefixes(lx, oracle, cls):
+    """The prefix map of a DF launch with RAGGED, short prefixes: hand-made screening factors (any positive numbers are legal
+    inputs of the schedule) leave 0..6 aux shells per pair, so that one batch of 32 sets spans a dozen and more pairs and the
+    pairs at the tail of a bucket have no set at all — the warp-cooperative pair search (find_pair_warp) and the run-wise J
+    reduction against the oracle, which screens with the same numbers.  Set counts are bit-exact."""
+    from helpers import table
+    lxa, la, lb = cls
+    rng = np.random.default_rng(900 + 100 * lxa + 10 * la + lb)
+    nsh = 30
+    shells = []
+    for i in range(2 * nsh):
+        l = la if i < nsh else lb
+        k = int(rng.integers(1, 3))
+        z = np.exp(rng.uniform(np.log(0.3), np.log(2.5), k))
+        shells.append((l, rng.uniform(0, 5, 3), z, rng.uniform(0.3, 1.0, k) * gen.prim_norm(z, l)))
+    prim = table(shells)
+    xs = []
+    for _ in range(6):
+        z = np.exp(rng.uniform(np.log(0.3), np.log(2.5), 1))
+        xs.append((lxa, rng.uniform(0, 5, 3), z, gen.prim_norm(z, lxa)))
+    aux = table(xs)
+    # every (la-shell, lb-shell) pair: 900 pairs of one class
+    pairs = np.array([[i, nsh + j] for i in range(nsh) for j in range(nsh)], np.int32)
+    qx = 10.0 ** -np.arange(6, dtype=np.float64)                      # 1, 0.1, ... 1e-5
+    qp = 10.0 ** -rng.uniform(0.0, 8.0, len(pairs))
+    tau = 1e-6
+    D = rng.normal(size=(prim.nbf, prim.nbf))
+    D = D + D.T
+    d = rng.normal(size=aux.nbf)
+    g_ref, J_ref, nsets, nints = oracle.df_gamma_J(aux, prim, pairs, qx, qp, tau, D=D, d=d)
+    sched, gamma, J = _gpu_df(lx, aux, prim, pairs, qx, qp, tau, D, d)
+    assert sched.num_sets == nsets and sched.num_integrals == nints
+    assert 1.5 * len(pairs) < nsets < 4.5 * len(pairs)                # a few sets per pair on average
+    eg, eJ = _relerr(gamma, g_ref), _relerr(J, J_ref)
+    assert eg <= TOL_DF and eJ <= TOL_DF, (lx.lx_kernel_family(*cls), eg, eJ)
