@@ -47,8 +47,9 @@ struct SlabCls {
     static constexpr int UREC = O_CK + NLEV;
     // staging of one finished slab of a shell-set: the rows a (a_x = s) x all b; the largest is s = 0
     static constexpr int STG = (LA + 1) * NB;
-    // A TEAM of T warps owns a ket component: they share its (e0|c) region and split the slab groups and the HRR rows; each
-    // warp has its own staging slot.  Sets per batch: 32 where that leaves room for LX_SLAB_MINW32 warps, else 16 (lanes
+    // A TEAM of T warps owns a ket component and shares its (e0|c) region; T = 1 (one warp per component) since the chains
+    // run on the whole vector in one warp's registers; with LX_SLAB_TEAM = 2 the second warp only takes HRR rows (tuning knob).
+    // Each warp has its own staging slot.  Sets per batch: 32 where that leaves room for LX_SLAB_MINW32 warps, else 16 (lanes
     // 16..31 mirror 0..15).
     static constexpr int T = LX_SLAB_TEAM;
     static constexpr int per_team32 = (NACC + T * (STG | 1)) * 32 * 8, fixed32 = UREC * 32 * 8;
@@ -411,7 +412,7 @@ __device__ __forceinline__ void slab_item(int item, int q, const OwnHdr *h, doub
 // member of a team of T that takes item k of a list ordered by decreasing size ("snake": 0 1 .. T−1 T−1 .. 1 0)
 __host__ __device__ constexpr int snake(int k, int T) { return (k % (2 * T)) < T ? k % T : 2 * T - 1 - k % (2 * T); }
 
-// the slab groups team member wt runs for ket component c
+// the chains of ket component c (member 0 of the team)
 template <int LX, int LA, int LB>
 __device__ __forceinline__ void slab_component_chains(int c, int wt, const double *__restrict__ ub, int kprim,
                                                       double *__restrict__ e0t, int ls, bool add, double scale) {
