@@ -476,6 +476,75 @@ __device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, dou
     __syncthreads();
 }
 
+// Digestion straight from the registers of a solo team (W = 1) for Lx <= 1, where (e0|c) needs no gather: HRR (a7, eq. 1) per ket
+// component on the lane's accumulators, then a9 / a10 as in chain_epilogue — without the trip of the targets and the finished
+// shell-set through shared memory and without the three block barriers.  For the short batches of the low-L, weakly contracted DF
+// classes that trip is a quarter of the instructions of a batch (config 5: the Lx = 0, 1 team classes 318 -> see DESIGN.md §10).
+template <int LX, int LA, int LB, int MODE>
+__device__ __forceinline__ void direct_digest(const double *__restrict__ acc, const SetId &sid, int lane,
+                                              const DevShells &aux, const DevShells &prim, const DfArgs &df) {
+    using CC = ChainCls<LX, LA, LB>;
+    constexpr int NACC = CC::NACC, NXC = CC::NXC, NA = CC::NA, NB = CC::NB, NAB = CC::NAB;
+    constexpr unsigned FULL = 0xffffffffu;
+    static_assert(LX <= 1 && (MODE == 1 || MODE == 2), "level-0 targets only; DF modes");
+    double AB[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) AB[d] = prim.center[3 * sid.a + d] - prim.center[3 * sid.b + d];
+    if constexpr (MODE == 1) {
+        // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
+        const double *Dab = df.D + (size_t)prim.bf_off[sid.a] * df.ld + prim.bf_off[sid.b];
+        const double f = (sid.a != sid.b) ? 2.0 : 1.0;
+        double *gx = df.out + aux.bf_off[sid.x];
+        static_for<0, NXC>([&](auto ic) {
+            constexpr int c = decltype(ic)::value;
+            double H0[NACC], fin[NAB];
+            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = acc[c * NACC + decltype(ii)::value] * (double)cart_fact(off(LA) + decltype(ii)::value); });
+            hrr_store<LA, LB>(H0, AB, fin, false);
+            double sum = 0.0;
+            static_for<0, NA>([&](auto ia) {
+                static_for<0, NB>([&](auto ib) {
+                    sum = fma(fin[decltype(ia)::value * NB + decltype(ib)::value], __ldg(Dab + (size_t)decltype(ia)::value * df.ld + decltype(ib)::value), sum);
+                });
+            });
+            if (sid.live) atomicAdd(gx + c, f * sum);
+        });
+    } else {
+        // J[bf(a)+ia, bf(b)+ib] += Σ_X Σ_c (c|ab) d[bf(X)+c], mirrored: v[r] of the lane's set in registers, the lanes that share a
+        // shell pair (contiguous runs of the batch) summed by shuffles, one atomic per run and element
+        const double *dx = df.D + aux.bf_off[sid.x];
+        double v[NAB];
+#pragma unroll
+        for (int r = 0; r < NAB; ++r) v[r] = 0.0;
+        static_for<0, NXC>([&](auto ic) {
+            constexpr int c = decltype(ic)::value;
+            double H0[NACC], fin[NAB];
+            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = acc[c * NACC + decltype(ii)::value] * (double)cart_fact(off(LA) + decltype(ii)::value); });
+            hrr_store<LA, LB>(H0, AB, fin, false);
+            const double dc = sid.live ? __ldg(dx + c) : 0.0;
+            static_for<0, NAB>([&](auto ir) { v[decltype(ir)::value] = fma(fin[decltype(ir)::value], dc, v[decltype(ir)::value]); });
+        });
+        unsigned rest = __ballot_sync(FULL, sid.live);
+        while (rest) {                                        // warp-uniform loop over the runs of equal pairs
+            const int leader = __ffs(rest) - 1;
+            const int pl = __shfl_sync(FULL, sid.p, leader);
+            const unsigned grp = __ballot_sync(FULL, sid.live && sid.p == pl) & rest;
+            const bool in = (grp >> lane) & 1u;
+            const size_t ra0 = prim.bf_off[sid.a], rb0 = prim.bf_off[sid.b];
+            static_for<0, NAB>([&](auto ir) {
+                constexpr int r = decltype(ir)::value, ia = r / NB, ib = r - ia * NB;
+                double sum = in ? v[r] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+                if (lane == leader) {
+                    atomicAdd(df.out + (ra0 + ia) * df.ld + rb0 + ib, sum);
+                    if (sid.a != sid.b) atomicAdd(df.out + (rb0 + ib) * df.ld + ra0 + ia, sum);
+                }
+            });
+            rest &= ~grp;
+        }
+    }
+}
+
 // ---- team plan: W warps, warp w owns the targets [w·NTW, (w+1)·NTW) (ordered by level) ------------------------------------
 template <int LX, int LA, int LB, int W>
 struct TeamCls {
@@ -505,6 +574,8 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
     constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NT = MODE == 3 ? CC::NXC : TM::NT, NTW = (NT + W - 1) / W;
     constexpr int NUBX = MODE == 3 ? cmax(TM::NUB, 32 * (((2 * LX + 1) * CC::NAB) | 1)) : TM::NUB;   // staging / pure region
     constexpr unsigned FULL = 0xffffffffu;
+    // solo teams of the Lx <= 1 classes digest from registers in the DF modes (direct_digest)
+    constexpr bool DIRECT = W == 1 && LX <= 1 && (MODE == 1 || MODE == 2);
 
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]
@@ -574,13 +645,18 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
 #pragma unroll
                         for (int m = 0; m <= MHI - MLO; ++m) F[m] = Fn[m];
                     }
-                    static_for<T0, T1>([&](auto it) {
-                        constexpr int ti = decltype(it)::value;
-                        target_drop<LX, LA, LB>(ti, acc + (ti - T0) * NACC, TC, UB, lane);
-                    });
+                    if constexpr (DIRECT) {
+                        direct_digest<LX, LA, LB, MODE>(acc, sid, lane, aux, prim, df);
+                    } else {
+                        static_for<T0, T1>([&](auto it) {
+                            constexpr int ti = decltype(it)::value;
+                            target_drop<LX, LA, LB>(ti, acc + (ti - T0) * NACC, TC, UB, lane);
+                        });
+                    }
                 }
             }
         });
+        if constexpr (DIRECT) continue;                      // digested from registers: nothing went through shared memory
         __syncthreads();
         if constexpr (MODE == 3) pure_epilogue<LX, LA, LB, W>(TC, UB, df.D, warp, lane, batch, map, prim, out, swapped);
         else chain_epilogue<LX, LA, LB, MODE, W>(TC, UB, pt, warp, lane, batch, map, aux, prim, out, swapped, df, sid);
