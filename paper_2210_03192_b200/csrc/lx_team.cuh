@@ -476,7 +476,29 @@ __device__ __forceinline__ void pure_epilogue(const double *__restrict__ TC, dou
     __syncthreads();
 }
 
-// Digestion straight from the registers of a solo team (W = 1) for Lx <= 1, where (e0|c) needs no gather: HRR (a7, eq. 1) per ket
+// (e0|c)[i] = a_i! ( U_{0,c} + Σ_{n>0} β(c,n) U_{|n|,c−2n} )[i] from the accumulators of a lane that holds ALL targets of the class
+// (W = 1): the gather of chain_epilogue with the partner list resolved at compile time.
+template <int LX, int LA, int LB, int C_>
+__device__ __forceinline__ void e0c_from_acc(const double *__restrict__ acc, double (&H0)[ChainCls<LX, LA, LB>::NACC]) {
+    constexpr int NACC = ChainCls<LX, LA, LB>::NACC, gc = off(LX) + C_;
+    constexpr int cx = cart_pow(gc, 0), cy = cart_pow(gc, 1), cz = cart_pow(gc, 2);
+    static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = acc[C_ * NACC + decltype(ii)::value]; });
+    static_for<0, (cx / 2 + 1) * (cy / 2 + 1) * (cz / 2 + 1)>([&](auto in) {
+        constexpr int q = decltype(in)::value;
+        constexpr int nz = q % (cz / 2 + 1), ny = (q / (cz / 2 + 1)) % (cy / 2 + 1), nx = q / ((cz / 2 + 1) * (cy / 2 + 1));
+        if constexpr (nx + ny + nz > 0) {
+            constexpr int ti = target_index(LX, nx + ny + nz, cart_index(cx - 2 * nx, cy - 2 * ny, cz - 2 * nz));
+            constexpr double beta = (double)(beta1(cx, nx) * beta1(cy, ny) * beta1(cz, nz));
+            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = fma(beta, acc[ti * NACC + decltype(ii)::value], H0[decltype(ii)::value]); });
+        }
+    });
+    static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] *= (double)cart_fact(off(LA) + decltype(ii)::value); });
+}
+
+#ifndef LX_DIRECT_MAXLX
+#define LX_DIRECT_MAXLX 4
+#endif
+// Digestion straight from the registers of a solo team (W = 1): gather and HRR (a7, eq. 1) per ket
 // component on the lane's accumulators, then a9 / a10 as in chain_epilogue — without the trip of the targets and the finished
 // shell-set through shared memory and without the three block barriers.  For the short batches of the low-L, weakly contracted DF
 // classes that trip is a quarter of the instructions of a batch (config 5: the Lx = 0, 1 team classes 318 -> see DESIGN.md §10).
@@ -486,7 +508,7 @@ __device__ __forceinline__ void direct_digest(const double *__restrict__ acc, co
     using CC = ChainCls<LX, LA, LB>;
     constexpr int NACC = CC::NACC, NXC = CC::NXC, NA = CC::NA, NB = CC::NB, NAB = CC::NAB;
     constexpr unsigned FULL = 0xffffffffu;
-    static_assert(LX <= 1 && (MODE == 1 || MODE == 2), "level-0 targets only; DF modes");
+    static_assert(MODE == 1 || MODE == 2, "DF modes");
     double AB[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) AB[d] = prim.center[3 * sid.a + d] - prim.center[3 * sid.b + d];
@@ -498,7 +520,7 @@ __device__ __forceinline__ void direct_digest(const double *__restrict__ acc, co
         static_for<0, NXC>([&](auto ic) {
             constexpr int c = decltype(ic)::value;
             double H0[NACC], fin[NAB];
-            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = acc[c * NACC + decltype(ii)::value] * (double)cart_fact(off(LA) + decltype(ii)::value); });
+            e0c_from_acc<LX, LA, LB, c>(acc, H0);
             hrr_store<LA, LB>(H0, AB, fin, false);
             double sum = 0.0;
             static_for<0, NA>([&](auto ia) {
@@ -518,7 +540,7 @@ __device__ __forceinline__ void direct_digest(const double *__restrict__ acc, co
         static_for<0, NXC>([&](auto ic) {
             constexpr int c = decltype(ic)::value;
             double H0[NACC], fin[NAB];
-            static_for<0, NACC>([&](auto ii) { H0[decltype(ii)::value] = acc[c * NACC + decltype(ii)::value] * (double)cart_fact(off(LA) + decltype(ii)::value); });
+            e0c_from_acc<LX, LA, LB, c>(acc, H0);
             hrr_store<LA, LB>(H0, AB, fin, false);
             const double dc = sid.live ? __ldg(dx + c) : 0.0;
             static_for<0, NAB>([&](auto ir) { v[decltype(ir)::value] = fma(fin[decltype(ir)::value], dc, v[decltype(ir)::value]); });
@@ -574,8 +596,8 @@ team_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const doub
     constexpr int E = CC::E, NG = CC::NG, NACC = CC::NACC, NT = MODE == 3 ? CC::NXC : TM::NT, NTW = (NT + W - 1) / W;
     constexpr int NUBX = MODE == 3 ? cmax(TM::NUB, 32 * (((2 * LX + 1) * CC::NAB) | 1)) : TM::NUB;   // staging / pure region
     constexpr unsigned FULL = 0xffffffffu;
-    // solo teams of the Lx <= 1 classes digest from registers in the DF modes (direct_digest)
-    constexpr bool DIRECT = W == 1 && LX <= 1 && (MODE == 1 || MODE == 2);
+    // solo teams digest from registers in the DF modes (direct_digest)
+    constexpr bool DIRECT = W == 1 && LX <= LX_DIRECT_MAXLX && (MODE == 1 || MODE == 2);
 
     extern __shared__ double smem[];
     double *TC = smem;                                       // [set][c * NAB + ·]
