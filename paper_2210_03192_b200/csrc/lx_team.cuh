@@ -501,7 +501,8 @@ __device__ __forceinline__ void e0c_from_acc(const double *__restrict__ acc, dou
 // Digestion straight from the registers of a solo team (W = 1): gather and HRR (a7, eq. 1) per ket
 // component on the lane's accumulators, then a9 / a10 as in chain_epilogue — without the trip of the targets and the finished
 // shell-set through shared memory and without the three block barriers.  For the short batches of the low-L, weakly contracted DF
-// classes that trip is a quarter of the instructions of a batch (config 5: the Lx = 0, 1 team classes 318 -> see DESIGN.md §10).
+// classes that trip is a quarter of the instructions of a batch (config 5 DF-J 1.97 -> 1.87 s, config 4 9.0 -> 8.2 ms; the same
+// (3|10) launch 4.47 -> 3.92 ms, profiles/r02_ncu_team_df.md).
 template <int LX, int LA, int LB, int MODE>
 __device__ __forceinline__ void direct_digest(const double *__restrict__ acc, const SetId &sid, int lane,
                                               const DevShells &aux, const DevShells &prim, const DfArgs &df) {
