@@ -167,6 +167,7 @@ int lx_df_J(const lx_schedule_t *s, const lx_shells_t *aux, const lx_shells_t *p
  *   allocates: nothing — no cudaMalloc / cudaFree / allocating library routine; lx_init(device), which must have been
  *              called, has looked up the array's device address.  The first launch of a class kernel in a process loads
  *              its code and sets its shared-memory attribute (CUDA lazy loading): run each class once before a capture.
+ *   checks:    the LX_CHECK=1 validation pass of lx_eri3_batch (it synchronises) is not run here; lx_async_status() works as usual.
  *   sharing:   every call uses the SAME array and leaves its contents behind.  Nothing in it has to start at zero: a call
  *              rewrites every record it reads.  Calls that overlap on the GPU (different streams, or another process
  *              thread) RACE on it: issue them on one stream, or order them with events.  lx_eri3_batch with caller

@@ -18,8 +18,6 @@
 // loop and the start vectors of the next batch made ahead was slower on contracted launches ((5|22) K = 25: 22.5 against
 // 19.6 ms) and, in the end, on K = 1 launches as well ((6|22): 1.75 against 1.54 ms); it was removed.
 #pragma once
-#include <cstdlib>
-
 #include "lx_team.cuh"
 
 namespace lx {
@@ -65,7 +63,7 @@ struct OwnHdr {
     int xo0[32], Kab[32], K[32], a[32], b[32], x[32], p[32];
     int tr[32];    // slab kernel: the set is stored transposed ([c][b][a]: mirrored class, or roles exchanged for La = Lb)
     int kmax;      // largest K of the batch (0: no live set)
-    int ready;     // (unused)
+    int ready;     // spare
     int next_c;    // next ket component of the batch to hand out (warps take components dynamically)
     int next_p;    // slab kernel: next producer work item
 };
@@ -216,13 +214,14 @@ __device__ __forceinline__ void owner_partners(int c, const double *__restrict__
 }
 
 // a7 + a8/a9/a10 of one finished ket component: HRR in registers (eq. 1), then the 32 sets leave through
-// the warp's staging slot as one coalesced run per set (MODE 0), are contracted with D into γ (MODE 1) or added to the
-// warp's partial J sums (MODE 2; `first`: the slot holds nothing yet).
+// the warp's staging slot as one coalesced run per set (MODE 0) or are contracted with D into γ (MODE 1).  (The J digestion
+// never comes here: it sums Σ_c d_c (e0|c) in the accumulator and transfers once per batch, owner2_kernel::j_reduce.)
 template <int LX, int LA, int LB, int MODE>
 __device__ __forceinline__ void owner_finish(int c, const double (&acc)[OwnCls<LX, LA, LB>::NACC], const OwnHdr *hd,
                                              double *__restrict__ stw, int lane, long long batch, const SetMap &map,
                                              const DevShells &aux, const DevShells &prim, double *__restrict__ out, bool tr,
-                                             const DfArgs &df, bool first) {
+                                             const DfArgs &df) {
+    static_assert(MODE == 0 || MODE == 1, "store and gamma modes");
     using OC = OwnCls<LX, LA, LB>;
     constexpr int NACC = OC::NACC, NXC = OC::NXC, NA = OC::NA, NB = OC::NB, NAB = OC::NAB, SP = OC::SP;
     double H0[NACC];
@@ -245,26 +244,16 @@ __device__ __forceinline__ void owner_finish(int c, const double (&acc)[OwnCls<L
     } else {
         double fin[NAB];
         hrr_store<LA, LB>(H0, AB, fin, false);
-        const bool live = hd->p[lane] >= 0;
-        const int xs = hd->x[lane];
-        if constexpr (MODE == 1) {
-            // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
-            if (live) {
-                const int sa = hd->a[lane], sb = hd->b[lane];
-                const double *Dab = df.D + (size_t)prim.bf_off[sa] * df.ld + prim.bf_off[sb];
-                double sum = 0.0;
+        // γ[bf(X)+c] += f Σ_ab (c|ab) D[bf(a)+ia, bf(b)+ib]
+        if (hd->p[lane] >= 0) {
+            const int sa = hd->a[lane], sb = hd->b[lane];
+            const double *Dab = df.D + (size_t)prim.bf_off[sa] * df.ld + prim.bf_off[sb];
+            double sum = 0.0;
 #pragma unroll
-                for (int ia = 0; ia < NA; ++ia)
+            for (int ia = 0; ia < NA; ++ia)
 #pragma unroll
-                    for (int ib = 0; ib < NB; ++ib) sum = fma(fin[ia * NB + ib], __ldg(Dab + (size_t)ia * df.ld + ib), sum);
-                atomicAdd(df.out + aux.bf_off[xs] + c, (sa != sb ? 2.0 : 1.0) * sum);
-            }
-        } else {
-            // partial sums of this warp: JS[set][ab] += (c|ab) d[bf(X)+c]; reduced over warps and lanes at the end of the batch
-            const double dc = live ? __ldg(df.D + aux.bf_off[xs] + c) : 0.0;
-            double *js = stw + (size_t)lane * SP;
-#pragma unroll
-            for (int i = 0; i < NAB; ++i) js[i] = first ? fin[i] * dc : fma(fin[i], dc, js[i]);
+                for (int ib = 0; ib < NB; ++ib) sum = fma(fin[ia * NB + ib], __ldg(Dab + (size_t)ia * df.ld + ib), sum);
+            atomicAdd(df.out + aux.bf_off[hd->x[lane]] + c, (sa != sb ? 2.0 : 1.0) * sum);
         }
     }
 }
@@ -456,7 +445,7 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
                     for (int q = 0; q < kq; ++q) owner_partners<LX, LA, LB, false>(c, ub0 + (size_t)q * UB, lane, acc, scale);
                 }
                 if constexpr (MODE != 2) {
-                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df, false);
+                    owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, batch, map, aux, prim, out, tr, df);
 #pragma unroll
                     for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
                 }
@@ -499,7 +488,7 @@ owner2_kernel(SetMap map, DevShells aux, DevShells prim, PairData pdat, const do
                 }
                 if constexpr (MODE == 0 && NSLOT_C > NSLOT) __syncthreads();   // the staging slots overlap the buffers of the last chunk
                 if constexpr (MODE != 2) {
-                    if (c < NXC) owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df, false);
+                    if (c < NXC) owner_finish<LX, LA, LB, MODE>(c, acc, hd, stw, lane, base, map, aux, prim, out, tr, df);
 #pragma unroll
                     for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
                 }
