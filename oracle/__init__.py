@@ -7,4 +7,5 @@ product package and shares no code with the CUDA path.
 """
 from .lxo import (  # noqa: F401
     build, boys, boys_ld, eri3_batch, schwarz_aux, schwarz_pair, df_gamma_J, max_threads, ncart, components,
+    metric_2c, fit_solve,
 )

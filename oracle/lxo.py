@@ -155,3 +155,47 @@ def df_gamma_J(aux, prim, pair_idx, q_aux, q_pair, tau, D=None, d=None, x_sel=No
        _p(ps, i32) if ps is not None else null_i, C.c_int(len(ps) if ps is not None else 0),
        C.byref(nsets), C.byref(nints))
     return gamma, J, int(nsets.value), int(nints.value)
+
+
+class _Tab:
+    pass
+
+
+def metric_2c(aux):
+    """Two-centre Coulomb metric of the fit, V[bf(X)+c, bf(Y)+c'] = (X_c|Y_c') = ∬ X_c(r1) Y_c'(r2) / r12 (PAPER.md:21,
+    :365 "the two-center ... integrals"), Cartesian components, [naux_bf, naux_bf] float64.
+
+    Written out from the definition with the 3-centre routine: Y_c'(r2) = Y_c'(r2) · 1 and the constant 1 is an s
+    Gaussian of exponent 0 and coefficient 1 (any centre), so (X|Y) = (X|Y 1) — eq. 12 with ζ_b = 0, where the product
+    centre P = A and the overlap factor is 1.  Pins: tests/test_oracle_metric.py (closed forms for s and p shells,
+    symmetry between the two routes (X|Y 1) and (Y|X 1), the diagonal against the separate Schwarz routine, positive
+    definiteness)."""
+    L = _i32(aux.L)
+    n = len(L)
+    ext = _Tab()
+    ext.L = np.concatenate([L, np.zeros(1, np.int32)])
+    po = _i32(aux.prim_off)
+    ext.prim_off = np.concatenate([po, np.asarray([po[-1] + 1], np.int32)])
+    ext.center = np.concatenate([_f64(aux.center).reshape(-1), np.zeros(3)])
+    ext.zeta = np.concatenate([_f64(aux.zeta), np.zeros(1)])
+    ext.coef = np.concatenate([_f64(aux.coef), np.ones(1)])
+    bf = _i32(aux.bf_off)
+    nbf = int(bf[-1])
+    V = np.zeros((nbf, nbf), dtype=np.float64)
+    for lx in sorted(set(L.tolist())):
+        xs = np.nonzero(L == lx)[0]
+        for ly in sorted(set(L.tolist())):
+            ys = np.nonzero(L == ly)[0]
+            out = eri3_batch(lx, ly, 0, aux, ext, xs, [[int(y), n] for y in ys])      # [ny, nx, nc(lx), nc(ly), 1]
+            for iy, y in enumerate(ys):
+                for ix, x in enumerate(xs):
+                    V[bf[x]:bf[x + 1], bf[y]:bf[y + 1]] = out[iy, ix, :, :, 0]
+    return V
+
+
+def fit_solve(V, gamma):
+    """Fit coefficients d = V⁻¹ γ (PAPER.md:21 robust fit, :365) by the LAPACK Cholesky
+    factorisation V = L Lᵀ and two triangular solves (numpy/scipy library routine as the step)."""
+    import scipy.linalg as sl
+    c = sl.cho_factor(np.asarray(V, dtype=np.float64), lower=True)
+    return sl.cho_solve(c, np.asarray(gamma, dtype=np.float64))
