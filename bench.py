@@ -311,6 +311,38 @@ def bench_df(lx, dev, costmodel, cfg, name, reps, unscreened=False):
     e2e = {"df_j_ms": e2e_ms, "integrals_per_s": 2 * sched.num_integrals / (e2e_ms * 1e-3),
            "h2d_bytes": int(D_h.numel() * 8 + d_h.numel() * 8), "d2h_bytes": int(g_h.numel() * 8 + J_h.numel() * 8),
            "note": "wall clock: H2D of D and d from pinned memory, lx_df_gamma, lx_df_J, D2H of gamma and J, synchronise"}
+    # the steps between the two passes: metric V = (X|Y) and its Cholesky factor once per basis,
+    # d = V^-1 gamma once per iteration (here: on the gamma of pass 1; the timed J pass above uses the synthetic d)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    V = lx.lx_metric_2c(ha)
+    t_met = time.perf_counter() - t0
+    fit = {"naux": aux.nbf, "metric_s": t_met, "metric_integrals_per_s": aux.nbf * (aux.nbf + 1) / 2 / t_met,
+           "note": "lx_metric_2c (own kernel, one thread per aux shell pair) on the whole aux basis; lx_fit_solve (cuSOLVER "
+                   "potrf / potrs) on the conditioned subset lx_inputs.fit_subset (the synthetic basis with its zeta = 0.1 "
+                   "shells is numerically singular, DESIGN.md); wall clock; once-per-basis steps except solve_ms"}
+    sub, keep = gen.fit_subset(aux)
+    keep = torch.as_tensor(keep, device=dev)
+    Vs = V[keep][:, keep].contiguous()
+    del V
+    gs = gam[keep].contiguous()
+    try:
+        t0 = time.perf_counter()
+        lx.lx_fit_solve(Vs, None)
+        fit["cholesky_s"] = time.perf_counter() - t0
+        dfit = gs.clone()
+        lx.lx_fit_solve(Vs, dfit, factored=True)
+        t_sol = []
+        for _ in range(max(1, reps)):
+            dfit.copy_(gs)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            lx.lx_fit_solve(Vs, dfit, factored=True)
+            t_sol.append((time.perf_counter() - t0) * 1e3)
+        fit.update({"naux_fit": sub.nbf, "solve_ms": min(t_sol)})
+    except lx.LxError as e:
+        fit["fit_error"] = str(e)
+    del Vs
     fl = _df_model_flops(costmodel, aux, prim, pairs, qx, qp, tau)
     floor_ms = fl / (FP64_NOMINAL_TFLOPS * 1e12) * 1e3
     res = {"workload": name, "screening": f"Schwarz, tau = {tau:g}, factors made on the GPU (lx_schwarz_aux_host / lx_schwarz_pair_host)",
@@ -321,7 +353,7 @@ def bench_df(lx, dev, costmodel, cfg, name, reps, unscreened=False):
            "integrals_per_s": 2 * sched.num_integrals / ((mg + mj) * 1e-3),
            "fp64_floor_ms_per_pass_costmodel": floor_ms, "frac_of_fp64_floor": 2 * floor_ms / (mg + mj),
            "check_gamma_dot_d": lhs, "check_J_dot_D": rhs, "check_rel_diff": abs(lhs - rhs) / max(abs(lhs), 1e-300),
-           "schwarz_s": t_q, "schedule_s": t_s, "e2e": e2e}
+           "schwarz_s": t_q, "schedule_s": t_s, "e2e": e2e, "fit": fit}
     if unscreened:
         s0 = lx.Schedule(ha, hp, None, None, pairs, 0.0)
         ug, uj = run(s0)

@@ -43,6 +43,7 @@ extern "C" {
 #define LX_ECUDA (-4)         /* CUDA runtime error; text via lx_strerror(LX_ECUDA)                             */
 #define LX_ENOTINIT (-5)      /* lx_init() has not been called on this device                                   */
 #define LX_ELIMIT (-6)        /* problem larger than the fixed scratch of lx_eri3_batch_static                 */
+#define LX_ENOTPD (-7)        /* lx_fit_solve: the metric is not (numerically) positive definite                */
 
 /* Gaussian shell table, structure of arrays (a shell is a centre, exponents ζ, contraction
  * coefficients and l, over unnormalised primitives).  Immutable during a call. */
@@ -115,6 +116,31 @@ size_t lx_eri3_workspace_bytes(int lx, int la, int lb, int nx, int npair, int km
  * Errors: LX_EINVAL, LX_EUNSUPPORTED (L outside the compiled range), LX_ENOTINIT, LX_ECUDA. */
 int lx_schwarz_aux_host(const lx_shells_t *aux_host, double *q_aux_host);
 int lx_schwarz_pair_host(const lx_shells_t *prim_host, const int32_t *pair_idx_host, int npair, double *q_pair_host);
+
+/* The steps after gamma and before J (SURVEY.md §8(f) NEXT-2, second half; PAPER.md:21 "robust" fit, :365 the two passes
+ * of density fitting):  V_XY = (X|Y) two-centre Coulomb metric of the aux basis,  d = V^-1 gamma  fit coefficients.
+ *
+ * lx_metric_2c:  V[(bf(X)+c)*ld + bf(Y)+c'] = (X_c|Y_c') = ∬ X_c(r1) Y_c'(r2) / r12  for every pair of aux shells, Cartesian
+ *   components in the library's order, bf(X) = Σ_{X'<X} nc(L_X') (aux_host->bf_off, if given, must say the same).
+ *   aux_host: HOST shell table (uploaded inside; L <= LX_MAX_L_AUX, any contraction degree).  V_dev: DEVICE, caller-owned,
+ *   [naux_bf rows, leading dimension ld >= naux_bf]; every entry of the naux_bf x naux_bf block is written (nothing has to
+ *   be cleared) and the result is exactly symmetric.  Evaluated by Hermite expansion of each shell about its own centre
+ *   (one thread per shell pair; lx_schwarz.cu), the same route as the Schwarz factors.  Synchronous.
+ *   Errors: LX_ENOTINIT, LX_EINVAL (null table / V_dev, ld too small, bf_off not Cartesian-cumulative, K inconsistent),
+ *   LX_EUNSUPPORTED (L out of range), LX_ECUDA.
+ *
+ * lx_fit_solve:  rhs <- V^-1 rhs by Cholesky factorisation (V = L L^T) and two triangular solves.
+ *   V_dev: DEVICE [n, ld], symmetric positive definite; OVERWRITTEN: one triangle holds the factor afterwards (the other
+ *   keeps V).  With factored != 0 the array is taken to hold that factor already (an earlier call on the same V) and only
+ *   the solves run — the usual case of one metric and a new gamma per SCF iteration.  rhs_dev: DEVICE, nrhs vectors of
+ *   length n, each contiguous (vector r at rhs_dev + r*n), overwritten by the solutions; nrhs = 0 only factorises.
+ *   The factorisation is cuSOLVER's potrf (a plain library routine, opened with dlopen at the first call); the triangular
+ *   solves are kernels of this library (lx_fit.cu: blocked substitution, 2 n/64 launches per right-hand side, the factor
+ *   read once each way).  Synchronous; allocates the factorisation workspace / n+65 doubles for the duration of the call.
+ *   Errors: LX_ENOTINIT, LX_EINVAL, LX_ENOTPD (a leading minor of V is not positive definite: linearly dependent aux
+ *   functions), LX_EUNSUPPORTED (factorising call and cuSOLVER cannot be loaded), LX_ENOMEM, LX_ECUDA. */
+int lx_metric_2c(const lx_shells_t *aux_host, double *V_dev, long long ld);
+int lx_fit_solve(double *V_dev, long long ld, int n, double *rhs_dev, int nrhs, int factored);
 
 /* Schedule — SURVEY.md §8(a) row a0; PAPER.md:54 (batches per class), :365 ("identical screening").
  * Built once per basis on the HOST from host copies of the shell tables.  Buckets aux shells by L and shell pairs

@@ -225,3 +225,17 @@ def config4(seed=4, natom=64):
 def config5(seed=5, natom=256):
     """256-atom cluster, 50-bohr box: primary 4s3p2d1f (first s K=10); aux 8s6p5d4f3g2h1i."""
     return _df_config(seed, natom, 50.0, _PRIM5, _AUX5)
+
+
+def fit_subset(aux, zmin=0.15):
+    """The aux shells usable as a FIT basis: the synthetic aux sets of configs 4/5 put ζ = 0.1 functions of every L on
+    every atom, which makes the two-centre metric numerically singular (config 4: λmin/λmax = 7e-19 by the oracle);
+    without the shells of smallest exponent < zmin the condition number is ~1e8.  Returns (table of the kept shells,
+    basis-function indices of the kept shells in the full table)."""
+    keep = [i for i in range(aux.nshell) if float(np.min(aux.zeta[aux.prim_off[i]:aux.prim_off[i + 1]])) >= zmin]
+    ctr = aux.center.reshape(-1, 3)
+    sub = make_shells([aux.L[i] for i in keep], [ctr[i] for i in keep],
+                      [aux.zeta[aux.prim_off[i]:aux.prim_off[i + 1]] for i in keep],
+                      [aux.coef[aux.prim_off[i]:aux.prim_off[i + 1]] for i in keep])
+    idx = np.concatenate([np.arange(aux.bf_off[i], aux.bf_off[i + 1]) for i in keep]) if keep else np.zeros(0, np.int64)
+    return sub, idx

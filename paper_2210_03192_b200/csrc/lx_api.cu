@@ -320,6 +320,7 @@ const char *lx_strerror(int status) {
         case LX_ECUDA: return g.cuda_msg;
         case LX_ENOTINIT: return "lx_init() has not been called";
         case LX_ELIMIT: return "npair * kmax_pair exceeds the fixed scratch of lx_eri3_batch_static (LX_STATIC_SCRATCH_BYTES = 4 MiB = 87381 primitive pairs): use lx_eri3_batch with a workspace";
+        case LX_ENOTPD: return "lx_fit_solve: the metric is not positive definite (linearly dependent aux functions?)";
         default: return "unknown status";
     }
 }

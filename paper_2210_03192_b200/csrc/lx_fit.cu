@@ -1,0 +1,203 @@
+// lx_fit.cu — the fit solve d = V⁻¹ γ of density fitting (second half):
+// Cholesky factorisation V = L Lᵀ of the two-centre metric and two triangular solves per right-hand side.
+//
+// The factorisation is a dense LAPACK routine (potrf), not part of the integral path, and is taken from cuSOLVER as a
+// plain library call (like a library GEMM would be).  cuSOLVER is opened at the first call with dlopen, so that liblx.so
+// itself has no link-time dependency on it: where the library is missing, a factorising call returns LX_EUNSUPPORTED and
+// every other entry point works as before.
+//
+// The two triangular solves — the part that runs every iteration — are kernels of this file: the library's potrs treats a
+// single right-hand side as a matrix (trsm) and took 0.79 s at n = 39 680 where the factor is only read once each way
+// (2 x 6.3 GB).  Layout: potrf(LOWER) on the column-major image of the symmetric array leaves, in ROW-major terms, the upper
+// triangle U = Lᵀ (U[i][j], j >= i, rows contiguous), V = Uᵀ U.
+//   forward   Uᵀ y = g : block column by block column (64 wide): every CTA solves the 64 x 64 diagonal block in shared
+//             memory (redundantly: cheaper than a second launch), then subtracts the block's contribution from its 256
+//             later entries of g — rows of U read along j, coalesced.
+//   backward  U d = y  : block row by block row from the end: one CTA per row takes the dot product with the part of d
+//             already known (the row is contiguous), the last CTA to finish (ticket) solves the diagonal block.
+// 2 n/64 launches per right-hand side, each reading its rows of the factor exactly once.
+#include <cusolverDn.h>
+#include <dlfcn.h>
+
+#include <mutex>
+
+#include "../../include/lx.h"
+#include "lx_state.h"
+
+namespace {
+
+struct Solver {
+    bool tried = false, ok = false;
+    void *so = nullptr;
+    decltype(&cusolverDnCreate) create = nullptr;
+    decltype(&cusolverDnDestroy) destroy = nullptr;
+    decltype(&cusolverDnCreateParams) create_params = nullptr;
+    decltype(&cusolverDnDestroyParams) destroy_params = nullptr;
+    decltype(&cusolverDnXpotrf_bufferSize) potrf_size = nullptr;
+    decltype(&cusolverDnXpotrf) potrf = nullptr;
+    cusolverDnHandle_t handle = nullptr;      // made once, kept for the life of the process
+
+    template <class F>
+    bool sym(F &f, const char *name) {
+        f = reinterpret_cast<F>(dlsym(so, name));
+        return f != nullptr;
+    }
+    bool load() {
+        if (tried) return ok;
+        tried = true;
+        for (const char *n : {"libcusolver.so.11", "libcusolver.so.12", "libcusolver.so"}) {
+            so = dlopen(n, RTLD_NOW | RTLD_GLOBAL);
+            if (so) break;
+        }
+        if (!so) return false;
+        ok = sym(create, "cusolverDnCreate") && sym(destroy, "cusolverDnDestroy") &&
+             sym(create_params, "cusolverDnCreateParams") && sym(destroy_params, "cusolverDnDestroyParams") &&
+             sym(potrf_size, "cusolverDnXpotrf_bufferSize") && sym(potrf, "cusolverDnXpotrf");
+        if (ok && create(&handle) != CUSOLVER_STATUS_SUCCESS) ok = false;
+        return ok;
+    }
+};
+
+constexpr int TB = 64;       // block width of the triangular solves
+constexpr int TT = 256;      // threads per CTA
+
+// forward step of block column j0: y[j0..j0+m) from r, then r[j] -= Σ_i U[j0+i][j] y[j0+i] for j >= j0+m.
+__global__ void __launch_bounds__(TT)
+tri_fwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, double *__restrict__ r, double *__restrict__ y) {
+    __shared__ double Us[TB][TB + 1];
+    __shared__ double ys[TB];
+    const int m = min(TB, n - j0), tid = threadIdx.x;
+    for (int e = tid; e < TB * TB; e += TT) {
+        const int i = e / TB, j = e - i * TB;
+        Us[i][j] = (j >= i && j < m) ? U[(long long)(j0 + i) * ld + j0 + j] : 0.0;
+    }
+    double rj = tid < m ? r[j0 + tid] : 0.0;        // r[j0..j0+m) is not written by this launch
+    __syncthreads();
+    for (int i = 0; i < m; ++i) {
+        if (tid == i) ys[i] = rj / Us[i][i];
+        __syncthreads();
+        if (tid > i && tid < m) rj = fma(-Us[i][tid], ys[i], rj);
+    }
+    if (blockIdx.x == 0 && tid < m) y[j0 + tid] = ys[tid];
+    const long long j = (long long)j0 + m + (long long)blockIdx.x * TT + tid;
+    if (j < n) {
+        const double *col = U + (long long)j0 * ld + j;
+        double s0 = 0.0, s1 = 0.0;
+        int i = 0;
+        for (; i + 1 < m; i += 2) {
+            s0 = fma(col[(long long)i * ld], ys[i], s0);
+            s1 = fma(col[(long long)(i + 1) * ld], ys[i + 1], s1);
+        }
+        if (i < m) s0 = fma(col[(long long)i * ld], ys[i], s0);
+        r[j] -= s0 + s1;
+    }
+}
+
+// backward step of block row j0: t[i] = y[j0+i] − Σ_{j >= j0+m} U[j0+i][j] d[j] (one CTA per row), then the last CTA solves
+// the diagonal block for d[j0..j0+m).
+__global__ void __launch_bounds__(TT)
+tri_bwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, const double *__restrict__ y, double *d,
+               double *t, unsigned *ticket) {
+    __shared__ double Us[TB][TB + 1];
+    __shared__ double ds[TB];
+    __shared__ double red[TT / 32];
+    __shared__ bool last;
+    const int m = min(TB, n - j0), tid = threadIdx.x, i = blockIdx.x;
+    const double *row = U + (long long)(j0 + i) * ld;
+    double s = 0.0;
+    for (long long j = (long long)j0 + m + tid; j < n; j += TT) s = fma(row[j], d[j], s);
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((tid & 31) == 0) red[tid >> 5] = s;
+    __syncthreads();
+    if (tid == 0) {
+        double a = 0.0;
+        for (int w = 0; w < TT / 32; ++w) a += red[w];
+        t[i] = y[j0 + i] - a;
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == (unsigned)(m - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (int e = tid; e < TB * TB; e += TT) {
+        const int a = e / TB, b = e - a * TB;
+        Us[a][b] = (b >= a && b < m) ? U[(long long)(j0 + a) * ld + j0 + b] : 0.0;
+    }
+    double tk = tid < m ? __ldcg(t + tid) : 0.0;
+    if (tid == 0) *ticket = 0u;                      // ready for the next launch (stream order)
+    __syncthreads();
+    for (int c = m - 1; c >= 0; --c) {
+        if (tid == c) ds[c] = tk / Us[c][c];
+        __syncthreads();
+        if (tid < c) tk = fma(-Us[tid][c], ds[c], tk);
+    }
+    if (tid < m) d[j0 + tid] = ds[tid];
+}
+
+Solver g_solver;
+std::mutex g_mu;
+
+}  // namespace
+
+extern "C" int lx_fit_solve(double *V_dev, long long ld, int n, double *rhs_dev, int nrhs, int factored) {
+    if (!lx::state_ready()) return LX_ENOTINIT;
+    if (n < 0 || nrhs < 0 || ld < n) return LX_EINVAL;
+    if (n == 0) return LX_OK;
+    if (!V_dev || (nrhs > 0 && !rhs_dev)) return LX_EINVAL;
+    std::lock_guard<std::mutex> lock(g_mu);
+    int rc = LX_OK;
+    void *dwork = nullptr, *hwork = nullptr;
+    double *scratch = nullptr;
+    int *dinfo = nullptr, info = 0;
+    auto cuda_ok = [&](cudaError_t e) {
+        if (e != cudaSuccess && rc == LX_OK) rc = lx::state_cuda_fail((int)e);
+        return e == cudaSuccess;
+    };
+    do {
+        if (!factored) {
+            if (!g_solver.load()) { rc = LX_EUNSUPPORTED; break; }
+            cusolverDnParams_t prm = nullptr;
+            bool ok = g_solver.create_params(&prm) == CUSOLVER_STATUS_SUCCESS;
+            // V is symmetric: its row-major image is its column-major image
+            const cublasFillMode_t uplo = CUBLAS_FILL_MODE_LOWER;
+            size_t dbytes = 0, hbytes = 0;
+            ok = ok && g_solver.potrf_size(g_solver.handle, prm, uplo, n, CUDA_R_64F, V_dev, ld, CUDA_R_64F, &dbytes, &hbytes) ==
+                           CUSOLVER_STATUS_SUCCESS;
+            if (ok) ok = cuda_ok(cudaMalloc((void **)&dinfo, sizeof(int))) && (!dbytes || cuda_ok(cudaMalloc(&dwork, dbytes)));
+            if (ok && hbytes && !(hwork = malloc(hbytes))) { rc = LX_ENOMEM; ok = false; }
+            ok = ok && g_solver.potrf(g_solver.handle, prm, uplo, n, CUDA_R_64F, V_dev, ld, CUDA_R_64F, dwork, dbytes, hwork,
+                                      hbytes, dinfo) == CUSOLVER_STATUS_SUCCESS;
+            ok = ok && cuda_ok(cudaMemcpy(&info, dinfo, sizeof(int), cudaMemcpyDeviceToHost));
+            if (prm) g_solver.destroy_params(prm);
+            if (!ok) { if (rc == LX_OK) rc = lx::state_cuda_fail((int)cudaErrorUnknown); break; }
+            if (info != 0) { rc = LX_ENOTPD; break; }                // a leading minor is not positive definite
+        }
+        if (nrhs > 0) {
+            // y [n] | t [TB] | ticket
+            if (!cuda_ok(cudaMalloc((void **)&scratch, ((size_t)n + TB + 1) * sizeof(double)))) break;
+            double *y = scratch, *t = scratch + n;
+            unsigned *ticket = reinterpret_cast<unsigned *>(scratch + n + TB);
+            if (!cuda_ok(cudaMemset(ticket, 0, sizeof(double)))) break;
+            const int nb = (n + TB - 1) / TB;
+            for (int r = 0; r < nrhs; ++r) {
+                double *g = rhs_dev + (size_t)r * n;
+                for (int b = 0; b < nb; ++b) {
+                    const int j0 = b * TB, m = n - j0 < TB ? n - j0 : TB, rest = n - j0 - m;
+                    tri_fwd_kernel<<<rest > 0 ? (rest + TT - 1) / TT : 1, TT>>>(V_dev, ld, n, j0, g, y);
+                }
+                for (int b = nb - 1; b >= 0; --b) {
+                    const int j0 = b * TB, m = n - j0 < TB ? n - j0 : TB;
+                    tri_bwd_kernel<<<m, TT>>>(V_dev, ld, n, j0, y, g, t, ticket);
+                }
+            }
+            lx::state_count_launches(2 * nb * nrhs);
+            if (!cuda_ok(cudaGetLastError())) break;
+        }
+        cuda_ok(cudaDeviceSynchronize());
+    } while (false);
+    cudaFree(dwork);
+    cudaFree(dinfo);
+    cudaFree(scratch);
+    free(hwork);
+    return rc;
+}

@@ -1,4 +1,5 @@
-// lx_schwarz.cu — Schwarz factors on the GPU (first half; "identical screening"):
+// lx_schwarz.cu — Schwarz factors and the two-centre metric V_XY = (X|Y) on the GPU (PAPER.md:365
+// "identical screening", :21 the fit metric):
 //     Q_X  = sqrt(max_c (X_c|X_c))          2-centre Coulomb integrals of an aux shell with itself
 //     Q_ab = sqrt(max_{a,b} (a b|a b))      diagonal 4-centre integrals of a primary shell pair
 // so that |(X|ab)| <= Q_X Q_ab for every component and a shell-set with Q_X Q_ab < tau can be skipped.
@@ -209,6 +210,83 @@ schwarz_aux_kernel(DevShells aux, const int32_t *__restrict__ ids, int n, const 
     q[x] = sqrt(mx);
 }
 
+// ---- two-centre metric V_XY = (X|Y) (second half) -----------------------------
+// One thread per pair of aux shells (X of angular momentum LX, Y of LY <= LX; for LX = LY only y <= x), all Cartesian
+// components of the block in local memory.  A single Gaussian about its own centre has E_t^{i0} = 0 unless t ≡ i (mod 2)
+// (PA = 0 in the recurrence), so the Hermite sums step by two.  The block and its transpose are written, the diagonal
+// block (x = y) symmetrised, so V is exactly symmetric.
+template <int LX, int LY>
+__global__ void __launch_bounds__(64)
+metric_kernel(DevShells aux, const int32_t *__restrict__ bf_off, const int32_t *__restrict__ idx, int nX,
+              const int32_t *__restrict__ idy, int nY, const double *__restrict__ boys_tab, double *__restrict__ V,
+              long long ld) {
+    constexpr int L = LX + LY, N1 = L + 1, NTX = LX + 1, NTY = LY + 1, NX = nc(LX), NY = nc(LY);
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (long long)nX * nY) return;
+    const int ix = (int)(k / nY), iy = (int)(k - (long long)ix * nY);
+    const int x = idx[ix], y = idy[iy];
+    if (LX == LY && y > x) return;
+    const int Kx = aux.K[x], Ky = aux.K[y], ox = aux.prim_off[x], oy = aux.prim_off[y];
+    double AB[3];
+    for (int d = 0; d < 3; ++d) AB[d] = aux.center[3 * x + d] - aux.center[3 * y + d];
+    double EX[(LX + 1) * NTX], EY[(LY + 1) * NTY], R[N1 * N1 * N1], blk[NX * NY];
+    for (int i = 0; i < NX * NY; ++i) blk[i] = 0.0;
+    for (int i = 0; i < Kx; ++i) {
+        const double z1 = aux.zeta[ox + i];
+        hermite_pair<LX, 0>(0.0, 0.0, 0.5 / z1, EX);
+        for (int j = 0; j < Ky; ++j) {
+            const double z2 = aux.zeta[oy + j];
+            hermite_pair<LY, 0>(0.0, 0.0, 0.5 / z2, EY);
+            hermite_coulomb<L>(boys_tab, z1 * z2 / (z1 + z2), AB, R);
+            // 2π^{5/2} / (ζ1 ζ2 sqrt(ζ1+ζ2))
+            const double cc = 34.98683665524972497 / (z1 * z2) * rsqrt(z1 + z2) * aux.coef[ox + i] * aux.coef[oy + j];
+            for (int cx = 0; cx < NX; ++cx) {
+                int px[3];
+                cart_powers(LX, cx, px);
+                const double *e1x = EX + px[0] * NTX, *e1y = EX + px[1] * NTX, *e1z = EX + px[2] * NTX;
+                for (int cy = 0; cy < NY; ++cy) {
+                    int py[3];
+                    cart_powers(LY, cy, py);
+                    const double *e2x = EY + py[0] * NTY, *e2y = EY + py[1] * NTY, *e2z = EY + py[2] * NTY;
+                    // (−1)^{t'+u'+v'} with t' ≡ py (mod 2) throughout: one sign for the whole component
+                    const double sg = ((py[0] + py[1] + py[2]) & 1) ? -1.0 : 1.0;
+                    double s = 0.0;
+                    for (int t = px[0] & 1; t <= px[0]; t += 2)
+                        for (int t2 = py[0] & 1; t2 <= py[0]; t2 += 2) {
+                            const double fx = e1x[t] * e2x[t2];
+                            double sy = 0.0;
+                            for (int u = px[1] & 1; u <= px[1]; u += 2)
+                                for (int u2 = py[1] & 1; u2 <= py[1]; u2 += 2) {
+                                    const double fy = e1y[u] * e2y[u2];
+                                    const double *Rr = R + ((t + t2) * N1 + (u + u2)) * N1;
+                                    double sz = 0.0;
+                                    for (int v = px[2] & 1; v <= px[2]; v += 2) {
+                                        double s2 = 0.0;
+                                        for (int v2 = py[2] & 1; v2 <= py[2]; v2 += 2) s2 = fma(e2z[v2], Rr[v + v2], s2);
+                                        sz = fma(e1z[v], s2, sz);
+                                    }
+                                    sy = fma(fy, sz, sy);
+                                }
+                            s = fma(fx, sy, s);
+                        }
+                    blk[cx * NY + cy] = fma(cc * sg, s, blk[cx * NY + cy]);
+                }
+            }
+        }
+    }
+    double *Vxy = V + (long long)bf_off[x] * ld + bf_off[y], *Vyx = V + (long long)bf_off[y] * ld + bf_off[x];
+    if (x == y) {
+        for (int cx = 0; cx < NX; ++cx)
+            for (int cy = 0; cy < NY; ++cy) Vxy[(long long)cx * ld + cy] = 0.5 * (blk[cx * NY + cy] + blk[cy * NY + cx]);
+    } else {
+        for (int cx = 0; cx < NX; ++cx)
+            for (int cy = 0; cy < NY; ++cy) {
+                Vxy[(long long)cx * ld + cy] = blk[cx * NY + cy];
+                Vyx[(long long)cy * ld + cx] = blk[cx * NY + cy];
+            }
+    }
+}
+
 template <class T>
 static cudaError_t upload(const T *host, size_t n, T **dev) {
     *dev = nullptr;
@@ -347,6 +425,56 @@ int lx_schwarz_pair_host(const lx_shells_t *prim, const int32_t *pair_idx, int n
     }
     cudaFree(dq);
     return rc;
+}
+
+int lx_metric_2c(const lx_shells_t *aux, double *V_dev, long long ld) {
+    if (!state_ready()) return LX_ENOTINIT;
+    if (!table_ok(aux)) return LX_EINVAL;
+    if (aux->nshell == 0) return LX_OK;
+    std::vector<int32_t> ids[LX_MAX_L_AUX + 1], bf((size_t)aux->nshell + 1);
+    bf[0] = 0;
+    for (int i = 0; i < aux->nshell; ++i) {
+        const int l = aux->L[i];
+        if (l < 0 || l > LX_MAX_L_AUX) return LX_EUNSUPPORTED;
+        if (aux->K[i] < 1 || aux->prim_off[i + 1] - aux->prim_off[i] != aux->K[i]) return LX_EINVAL;
+        ids[l].push_back(i);
+        bf[i + 1] = bf[i] + (l + 1) * (l + 2) / 2;
+        if (aux->bf_off && aux->bf_off[i] != bf[i]) return LX_EINVAL;        // the metric is laid out in Cartesian order
+    }
+    if (!V_dev || ld < bf[aux->nshell]) return LX_EINVAL;
+    DevTable t;
+    LXS_CUDA(t.put(aux));
+    int32_t *dbf = nullptr, *dids[LX_MAX_L_AUX + 1] = {};
+    cudaError_t e = upload(bf.data(), bf.size(), &dbf);
+    for (int l = 0; l <= LX_MAX_L_AUX && e == cudaSuccess; ++l) e = upload(ids[l].data(), ids[l].size(), &dids[l]);
+    int launches = 0;
+    for (int lx = 0; lx <= LX_MAX_L_AUX && e == cudaSuccess; ++lx)
+        for (int ly = 0; ly <= lx && e == cudaSuccess; ++ly) {
+            const long long n = (long long)ids[lx].size() * (long long)ids[ly].size();
+            if (!n) continue;
+            const unsigned blocks = (unsigned)((n + 63) / 64);
+            switch (lx * (LX_MAX_L_AUX + 1) + ly) {
+#define LXS_MET(A_, B_) case A_ * (LX_MAX_L_AUX + 1) + B_:                                                      \
+    metric_kernel<A_, B_><<<blocks, 64>>>(t.view(), dbf, dids[A_], (int)ids[A_].size(), dids[B_], (int)ids[B_].size(), \
+                                          state_boys_tab(), V_dev, ld);                                         \
+    break;
+                LXS_MET(0, 0)
+                LXS_MET(1, 0) LXS_MET(1, 1)
+                LXS_MET(2, 0) LXS_MET(2, 1) LXS_MET(2, 2)
+                LXS_MET(3, 0) LXS_MET(3, 1) LXS_MET(3, 2) LXS_MET(3, 3)
+                LXS_MET(4, 0) LXS_MET(4, 1) LXS_MET(4, 2) LXS_MET(4, 3) LXS_MET(4, 4)
+                LXS_MET(5, 0) LXS_MET(5, 1) LXS_MET(5, 2) LXS_MET(5, 3) LXS_MET(5, 4) LXS_MET(5, 5)
+                LXS_MET(6, 0) LXS_MET(6, 1) LXS_MET(6, 2) LXS_MET(6, 3) LXS_MET(6, 4) LXS_MET(6, 5) LXS_MET(6, 6)
+#undef LXS_MET
+            }
+            ++launches;
+            e = cudaGetLastError();
+        }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    state_count_launches(launches);
+    cudaFree(dbf);
+    for (int l = 0; l <= LX_MAX_L_AUX; ++l) cudaFree(dids[l]);
+    return e == cudaSuccess ? LX_OK : state_cuda_fail((int)e);
 }
 
 }  // extern "C"

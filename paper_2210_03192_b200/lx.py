@@ -17,14 +17,15 @@ if not os.path.exists(_SO):
                       "there is no CPU fallback")
 _lib = C.CDLL(_SO)
 
-LX_OK, LX_EINVAL, LX_EUNSUPPORTED, LX_ENOMEM, LX_ECUDA, LX_ENOTINIT, LX_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+LX_OK, LX_EINVAL, LX_EUNSUPPORTED, LX_ENOMEM, LX_ECUDA, LX_ENOTINIT, LX_ELIMIT, LX_ENOTPD = 0, -1, -2, -3, -4, -5, -6, -7
 LX_MAX_L_AUX, LX_MAX_L_PRIM = 6, 4
 
 EXPORTS = ["lx_init", "lx_finalize", "lx_strerror", "lx_version", "lx_eri3_batch", "lx_eri3_workspace_bytes",
            "lx_schedule_create", "lx_schedule_destroy", "lx_schedule_num_sets", "lx_schedule_num_integrals",
            "lx_df_workspace_bytes", "lx_df_gamma", "lx_df_J", "lx_eri3_batch_host", "lx_boys", "lx_launch_count", "lx_fp64_probe", "lx_kernel_family", "lx_kernel_family_k",
            "lx_cart_to_pure", "lx_solid_matrix", "lx_eri3_batch_pure", "lx_eri3_pure_workspace_bytes", "lx_async_status",
-           "lx_schwarz_aux_host", "lx_schwarz_pair_host", "lx_eri3_batch_static", "lx_static_scratch_bytes"]
+           "lx_schwarz_aux_host", "lx_schwarz_pair_host", "lx_eri3_batch_static", "lx_static_scratch_bytes",
+           "lx_metric_2c", "lx_fit_solve"]
 
 
 class lx_shells_t(C.Structure):
@@ -244,6 +245,35 @@ def lx_schwarz_pair_host(prim_host, pair_idx):
     q = np.zeros(len(pair_idx), dtype=np.float64)
     _check(_lib.lx_schwarz_pair_host(C.byref(prim_host.struct), pair_idx.ctypes.data, len(pair_idx), q.ctypes.data))
     return q
+
+
+_lib.lx_metric_2c.argtypes = [C.POINTER(lx_shells_t), C.c_void_p, C.c_longlong]
+_lib.lx_fit_solve.argtypes = [C.c_void_p, C.c_longlong, C.c_int, C.c_void_p, C.c_int, C.c_int]
+
+
+def lx_metric_2c(aux_host, V=None):
+    """Two-centre metric V[bf(X)+c, bf(Y)+c'] = (X_c|Y_c') of the aux basis on the current device; HostShells in,
+    float64 CUDA tensor [naux_bf, naux_bf] out (written into `V` if given; its row stride is the leading dimension)."""
+    n = int(sum((int(l) + 1) * (int(l) + 2) // 2 for l in aux_host.L))
+    if V is None:
+        V = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    assert V.is_cuda and V.dtype == torch.float64 and V.dim() == 2 and V.shape[0] >= n and V.stride(1) == 1
+    _check(_lib.lx_metric_2c(C.byref(aux_host.struct), V.data_ptr(), V.stride(0)))
+    return V
+
+
+def lx_fit_solve(V, rhs, factored=False):
+    """rhs <- V^-1 rhs in place (Cholesky; `V` [n, n] CUDA float64 is overwritten by its factor, `factored=True` reuses
+    it).  rhs: CUDA float64 [n] or [nrhs, n] contiguous (one right-hand side per row), or None to factorise only."""
+    n = V.shape[0]
+    assert V.is_cuda and V.dtype == torch.float64 and V.dim() == 2 and V.shape[1] >= n and V.stride(1) == 1
+    nrhs = 0
+    if rhs is not None:
+        assert rhs.is_cuda and rhs.dtype == torch.float64 and rhs.is_contiguous() and rhs.shape[-1] == n
+        nrhs = rhs.numel() // n if n else 0
+    _check(_lib.lx_fit_solve(V.data_ptr(), V.stride(0), n, rhs.data_ptr() if rhs is not None else None, nrhs,
+                             1 if factored else 0))
+    return rhs
 
 
 class Schedule:
