@@ -61,40 +61,86 @@ struct Solver {
 constexpr int TB = 64;       // block width of the triangular solves
 constexpr int TT = 256;      // threads per CTA
 
+// The 64 x 64 diagonal block in shared memory: upper triangle of U, unit diagonal in the padding of a ragged last block.
+__device__ __forceinline__ void load_diag(double (*Us)[TB + 1], const double *__restrict__ U, long long ld, int j0, int m,
+                                          int tid) {
+    for (int e = tid; e < TB * TB; e += TT) {
+        const int i = e / TB, j = e - i * TB;
+        Us[i][j] = (j >= i && j < m) ? U[(long long)(j0 + i) * ld + j0 + j] : (i == j ? 1.0 : 0.0);
+    }
+}
+
+// Diagonal solves by ONE warp, lane l holding entries l and l+32 in registers; the pivot value travels by shuffle, so a step
+// of the serial chain is multiply (by the reciprocal pivot) - shuffle - fma, with no block barrier.
+// forward: Uᵀ y = r  (y_i = r_i / U_ii, then r_j -= U_ij y_i for j > i)
+__device__ __forceinline__ void diag_fwd(const double (*Us)[TB + 1], double r0, double r1, double *ys, int lane) {
+    const double v0 = 1.0 / Us[lane][lane], v1 = 1.0 / Us[lane + 32][lane + 32];
+#pragma unroll 8
+    for (int i = 0; i < 32; ++i) {
+        const double yi = __shfl_sync(0xffffffffu, r0 * v0, i);
+        if (lane == i) ys[i] = yi;
+        if (lane > i) r0 = fma(-Us[i][lane], yi, r0);
+        r1 = fma(-Us[i][lane + 32], yi, r1);
+    }
+#pragma unroll 8
+    for (int i = 32; i < 64; ++i) {
+        const double yi = __shfl_sync(0xffffffffu, r1 * v1, i - 32);
+        if (lane == i - 32) ys[i] = yi;
+        if (lane + 32 > i) r1 = fma(-Us[i][lane + 32], yi, r1);
+    }
+}
+// backward: U d = t  (d_c = t_c / U_cc, then t_k -= U_kc d_c for k < c)
+__device__ __forceinline__ void diag_bwd(const double (*Us)[TB + 1], double t0, double t1, double *ds, int lane) {
+    const double v0 = 1.0 / Us[lane][lane], v1 = 1.0 / Us[lane + 32][lane + 32];
+#pragma unroll 8
+    for (int c = 63; c >= 32; --c) {
+        const double dc = __shfl_sync(0xffffffffu, t1 * v1, c - 32);
+        if (lane == c - 32) ds[c] = dc;
+        if (lane + 32 < c) t1 = fma(-Us[lane + 32][c], dc, t1);
+        t0 = fma(-Us[lane][c], dc, t0);
+    }
+#pragma unroll 8
+    for (int c = 31; c >= 0; --c) {
+        const double dc = __shfl_sync(0xffffffffu, t0 * v0, c);
+        if (lane == c) ds[c] = dc;
+        if (lane < c) t0 = fma(-Us[lane][c], dc, t0);
+    }
+}
+
 // forward step of block column j0: y[j0..j0+m) from r, then r[j] -= Σ_i U[j0+i][j] y[j0+i] for j >= j0+m.
 __global__ void __launch_bounds__(TT)
 tri_fwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, double *__restrict__ r, double *__restrict__ y) {
     __shared__ double Us[TB][TB + 1];
     __shared__ double ys[TB];
     const int m = min(TB, n - j0), tid = threadIdx.x;
-    for (int e = tid; e < TB * TB; e += TT) {
-        const int i = e / TB, j = e - i * TB;
-        Us[i][j] = (j >= i && j < m) ? U[(long long)(j0 + i) * ld + j0 + j] : 0.0;
-    }
-    double rj = tid < m ? r[j0 + tid] : 0.0;        // r[j0..j0+m) is not written by this launch
-    __syncthreads();
-    for (int i = 0; i < m; ++i) {
-        if (tid == i) ys[i] = rj / Us[i][i];
-        __syncthreads();
-        if (tid > i && tid < m) rj = fma(-Us[i][tid], ys[i], rj);
-    }
-    if (blockIdx.x == 0 && tid < m) y[j0 + tid] = ys[tid];
+    load_diag(Us, U, ld, j0, m, tid);
     const long long j = (long long)j0 + m + (long long)blockIdx.x * TT + tid;
+    const double rj = j < n ? r[j] : 0.0;
+    __syncthreads();
+    if (tid < 32) {                                  // r[j0..j0+m) is not written by this launch
+        const double r0 = tid < m ? r[j0 + tid] : 0.0, r1 = tid + 32 < m ? r[j0 + tid + 32] : 0.0;
+        diag_fwd(Us, r0, r1, ys, tid);
+    }
+    __syncthreads();
+    if (blockIdx.x == 0 && tid < m) y[j0 + tid] = ys[tid];
     if (j < n) {
         const double *col = U + (long long)j0 * ld + j;
-        double s0 = 0.0, s1 = 0.0;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
         int i = 0;
-        for (; i + 1 < m; i += 2) {
+        for (; i + 3 < m; i += 4) {
             s0 = fma(col[(long long)i * ld], ys[i], s0);
             s1 = fma(col[(long long)(i + 1) * ld], ys[i + 1], s1);
+            s2 = fma(col[(long long)(i + 2) * ld], ys[i + 2], s2);
+            s3 = fma(col[(long long)(i + 3) * ld], ys[i + 3], s3);
         }
-        if (i < m) s0 = fma(col[(long long)i * ld], ys[i], s0);
-        r[j] -= s0 + s1;
+        for (; i < m; ++i) s0 = fma(col[(long long)i * ld], ys[i], s0);
+        r[j] = rj - ((s0 + s1) + (s2 + s3));
     }
 }
 
 // backward step of block row j0: t[i] = y[j0+i] − Σ_{j >= j0+m} U[j0+i][j] d[j] (one CTA per row), then the last CTA solves
-// the diagonal block for d[j0..j0+m).
+// the diagonal block for d[j0..j0+m).  Every CTA loads the diagonal block up front (its latency hides behind the row loads;
+// which CTA finishes last is not known before).
 __global__ void __launch_bounds__(TT)
 tri_bwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, const double *__restrict__ y, double *d,
                double *t, unsigned *ticket) {
@@ -103,9 +149,16 @@ tri_bwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, const 
     __shared__ double red[TT / 32];
     __shared__ bool last;
     const int m = min(TB, n - j0), tid = threadIdx.x, i = blockIdx.x;
+    load_diag(Us, U, ld, j0, m, tid);
     const double *row = U + (long long)(j0 + i) * ld;
-    double s = 0.0;
-    for (long long j = (long long)j0 + m + tid; j < n; j += TT) s = fma(row[j], d[j], s);
+    double s0 = 0.0, s1 = 0.0;
+    long long j = (long long)j0 + m + tid;
+    for (; j + TT < n; j += 2 * TT) {
+        s0 = fma(row[j], d[j], s0);
+        s1 = fma(row[j + TT], d[j + TT], s1);
+    }
+    if (j < n) s0 = fma(row[j], d[j], s0);
+    double s = s0 + s1;
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if ((tid & 31) == 0) red[tid >> 5] = s;
     __syncthreads();
@@ -119,18 +172,12 @@ tri_bwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, const 
     __syncthreads();
     if (!last) return;
     __threadfence();
-    for (int e = tid; e < TB * TB; e += TT) {
-        const int a = e / TB, b = e - a * TB;
-        Us[a][b] = (b >= a && b < m) ? U[(long long)(j0 + a) * ld + j0 + b] : 0.0;
-    }
-    double tk = tid < m ? __ldcg(t + tid) : 0.0;
     if (tid == 0) *ticket = 0u;                      // ready for the next launch (stream order)
-    __syncthreads();
-    for (int c = m - 1; c >= 0; --c) {
-        if (tid == c) ds[c] = tk / Us[c][c];
-        __syncthreads();
-        if (tid < c) tk = fma(-Us[tid][c], ds[c], tk);
+    if (tid < 32) {
+        const double t0 = tid < m ? __ldcg(t + tid) : 0.0, t1 = tid + 32 < m ? __ldcg(t + tid + 32) : 0.0;
+        diag_bwd(Us, t0, t1, ds, tid);
     }
+    __syncthreads();
     if (tid < m) d[j0 + tid] = ds[tid];
 }
 
