@@ -136,7 +136,8 @@ int lx_schwarz_pair_host(const lx_shells_t *prim_host, const int32_t *pair_idx_h
  *   length n, each contiguous (vector r at rhs_dev + r*n), overwritten by the solutions; nrhs = 0 only factorises.
  *   The factorisation is cuSOLVER's potrf (a plain library routine, opened with dlopen at the first call); the triangular
  *   solves are kernels of this library (lx_fit.cu: blocked substitution, 2 n/64 launches per right-hand side, the factor
- *   read once each way).  Synchronous; allocates the factorisation workspace / n+65 doubles for the duration of the call.
+ *   read once each way).  Synchronous; allocates the factorisation workspace / about n + n/32 doubles for the duration of the
+ *   call.
  *   Errors: LX_ENOTINIT, LX_EINVAL, LX_ENOTPD (a leading minor of V is not positive definite: linearly dependent aux
  *   functions), LX_EUNSUPPORTED (factorising call and cuSOLVER cannot be loaded), LX_ENOMEM, LX_ECUDA. */
 int lx_metric_2c(const lx_shells_t *aux_host, double *V_dev, long long ld);

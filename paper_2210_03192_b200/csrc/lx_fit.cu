@@ -11,10 +11,11 @@
 // (2 x 6.3 GB).  Layout: potrf(LOWER) on the column-major image of the symmetric array leaves, in ROW-major terms, the upper
 // triangle U = Lᵀ (U[i][j], j >= i, rows contiguous), V = Uᵀ U.
 //   forward   Uᵀ y = g : block column by block column (64 wide): every CTA solves the 64 x 64 diagonal block in shared
-//             memory (redundantly: cheaper than a second launch), then subtracts the block's contribution from its 256
+//             memory (redundantly: cheaper than a second launch), then subtracts the block's contribution from its 128
 //             later entries of g — rows of U read along j, coalesced.
-//   backward  U d = y  : block row by block row from the end: one CTA per row takes the dot product with the part of d
-//             already known (the row is contiguous), the last CTA to finish (ticket) solves the diagonal block.
+//   backward  U d = y  : block row by block row from the end: the dot product of each row with the part of d already known
+//             is split over CTAs of 2 048 entries (the row is contiguous; 8 loads per thread, all in flight), the last CTA
+//             to finish (ticket) sums the partial results in a fixed order and solves the diagonal block.
 // 2 n/64 launches per right-hand side, each reading its rows of the factor exactly once.
 #include <cusolverDn.h>
 #include <dlfcn.h>
@@ -59,12 +60,13 @@ struct Solver {
 };
 
 constexpr int TB = 64;       // block width of the triangular solves
-constexpr int TT = 256;      // threads per CTA
+constexpr int TT = 256;      // threads per CTA, backward step
+constexpr int TF = 128;      // threads per CTA, forward step (64 loads are held in registers: 170 registers per thread)
 
 // The 64 x 64 diagonal block in shared memory: upper triangle of U, unit diagonal in the padding of a ragged last block.
 __device__ __forceinline__ void load_diag(double (*Us)[TB + 1], const double *__restrict__ U, long long ld, int j0, int m,
-                                          int tid) {
-    for (int e = tid; e < TB * TB; e += TT) {
+                                          int tid, int nthreads) {
+    for (int e = tid; e < TB * TB; e += nthreads) {
         const int i = e / TB, j = e - i * TB;
         Us[i][j] = (j >= i && j < m) ? U[(long long)(j0 + i) * ld + j0 + j] : (i == j ? 1.0 : 0.0);
     }
@@ -108,14 +110,23 @@ __device__ __forceinline__ void diag_bwd(const double (*Us)[TB + 1], double t0, 
 }
 
 // forward step of block column j0: y[j0..j0+m) from r, then r[j] -= Σ_i U[j0+i][j] y[j0+i] for j >= j0+m.
-__global__ void __launch_bounds__(TT)
+__global__ void __launch_bounds__(TF)
 tri_fwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, double *__restrict__ r, double *__restrict__ y) {
     __shared__ double Us[TB][TB + 1];
     __shared__ double ys[TB];
     const int m = min(TB, n - j0), tid = threadIdx.x;
-    load_diag(Us, U, ld, j0, m, tid);
-    const long long j = (long long)j0 + m + (long long)blockIdx.x * TT + tid;
+    load_diag(Us, U, ld, j0, m, tid, TF);
+    const long long j = (long long)j0 + m + (long long)blockIdx.x * TF + tid;
     const double rj = j < n ? r[j] : 0.0;
+    // the thread's 64 entries of the block row (8·ld bytes apart) are requested BEFORE the barrier and the diagonal solve:
+    // they do not depend on y, the barrier keeps ptxas from sinking them, and their latency hides behind the solve
+    const double *col = U + (long long)j0 * ld + (j < n ? j : (long long)j0);
+    const bool full = m == TB;
+    double v[TB];
+    if (full) {
+#pragma unroll
+        for (int i = 0; i < TB; ++i) v[i] = __ldcs(col + (long long)i * ld);
+    }
     __syncthreads();
     if (tid < 32) {                                  // r[j0..j0+m) is not written by this launch
         const double r0 = tid < m ? r[j0 + tid] : 0.0, r1 = tid + 32 < m ? r[j0 + tid + 32] : 0.0;
@@ -124,57 +135,70 @@ tri_fwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, double
     __syncthreads();
     if (blockIdx.x == 0 && tid < m) y[j0 + tid] = ys[tid];
     if (j < n) {
-        const double *col = U + (long long)j0 * ld + j;
         double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-        int i = 0;
-        for (; i + 3 < m; i += 4) {
-            s0 = fma(col[(long long)i * ld], ys[i], s0);
-            s1 = fma(col[(long long)(i + 1) * ld], ys[i + 1], s1);
-            s2 = fma(col[(long long)(i + 2) * ld], ys[i + 2], s2);
-            s3 = fma(col[(long long)(i + 3) * ld], ys[i + 3], s3);
+        if (full) {
+#pragma unroll
+            for (int i = 0; i < TB; i += 4) {
+                s0 = fma(v[i], ys[i], s0);
+                s1 = fma(v[i + 1], ys[i + 1], s1);
+                s2 = fma(v[i + 2], ys[i + 2], s2);
+                s3 = fma(v[i + 3], ys[i + 3], s3);
+            }
+        } else {
+            for (int i = 0; i < m; ++i) s0 = fma(col[(long long)i * ld], ys[i], s0);
         }
-        for (; i < m; ++i) s0 = fma(col[(long long)i * ld], ys[i], s0);
         r[j] = rj - ((s0 + s1) + (s2 + s3));
     }
 }
 
-// backward step of block row j0: t[i] = y[j0+i] − Σ_{j >= j0+m} U[j0+i][j] d[j] (one CTA per row), then the last CTA solves
-// the diagonal block for d[j0..j0+m).  Every CTA loads the diagonal block up front (its latency hides behind the row loads;
-// which CTA finishes last is not known before).
+// backward step of block row j0: CTA (i, c) takes chunk c (TC entries) of the dot product Σ_{j >= j0+m} U[j0+i][j] d[j] of row
+// i into part[i][c]; the last CTA to finish (ticket) forms t_i = y_i − Σ_c part[i][c] (fixed order) and solves the diagonal
+// block for d[j0..j0+m).  Every CTA loads the diagonal block up front (its latency hides behind the row loads; which CTA
+// finishes last is not known before).
+constexpr int TC = 8 * TT;   // entries of a row per CTA: 8 per thread, all requested at once
+
 __global__ void __launch_bounds__(TT)
 tri_bwd_kernel(const double *__restrict__ U, long long ld, int n, int j0, const double *__restrict__ y, double *d,
-               double *t, unsigned *ticket) {
+               double *part, int npart, unsigned *ticket) {
     __shared__ double Us[TB][TB + 1];
     __shared__ double ds[TB];
     __shared__ double red[TT / 32];
     __shared__ bool last;
-    const int m = min(TB, n - j0), tid = threadIdx.x, i = blockIdx.x;
-    load_diag(Us, U, ld, j0, m, tid);
+    const int m = min(TB, n - j0), tid = threadIdx.x, i = blockIdx.x, c = blockIdx.y;
+    load_diag(Us, U, ld, j0, m, tid, TT);
     const double *row = U + (long long)(j0 + i) * ld;
-    double s0 = 0.0, s1 = 0.0;
-    long long j = (long long)j0 + m + tid;
-    for (; j + TT < n; j += 2 * TT) {
-        s0 = fma(row[j], d[j], s0);
-        s1 = fma(row[j + TT], d[j + TT], s1);
+    const long long jb = (long long)j0 + m + (long long)c * TC + tid;
+    double a[8], b[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const long long j = jb + k * TT;
+        a[k] = j < n ? __ldcs(row + j) : 0.0;
+        b[k] = j < n ? d[j] : 0.0;
     }
-    if (j < n) s0 = fma(row[j], d[j], s0);
-    double s = s0 + s1;
+    __syncthreads();                                 // scheduling fence: ptxas otherwise sinks the loads between the FMAs
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s = fma(a[k], b[k], s);
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if ((tid & 31) == 0) red[tid >> 5] = s;
     __syncthreads();
     if (tid == 0) {
-        double a = 0.0;
-        for (int w = 0; w < TT / 32; ++w) a += red[w];
-        t[i] = y[j0 + i] - a;
+        double acc = 0.0;
+        for (int w = 0; w < TT / 32; ++w) acc += red[w];
+        part[i * npart + c] = acc;
         __threadfence();
-        last = atomicAdd(ticket, 1u) == (unsigned)(m - 1);
+        last = atomicAdd(ticket, 1u) == (unsigned)(m * gridDim.y - 1);
     }
     __syncthreads();
     if (!last) return;
     __threadfence();
     if (tid == 0) *ticket = 0u;                      // ready for the next launch (stream order)
     if (tid < 32) {
-        const double t0 = tid < m ? __ldcg(t + tid) : 0.0, t1 = tid + 32 < m ? __ldcg(t + tid + 32) : 0.0;
+        double t0 = tid < m ? y[j0 + tid] : 0.0, t1 = tid + 32 < m ? y[j0 + tid + 32] : 0.0;
+        for (int q = 0; q < (int)gridDim.y; ++q) {
+            if (tid < m) t0 -= __ldcg(part + tid * npart + q);
+            if (tid + 32 < m) t1 -= __ldcg(part + (tid + 32) * npart + q);
+        }
         diag_bwd(Us, t0, t1, ds, tid);
     }
     __syncthreads();
@@ -220,21 +244,23 @@ extern "C" int lx_fit_solve(double *V_dev, long long ld, int n, double *rhs_dev,
             if (info != 0) { rc = LX_ENOTPD; break; }                // a leading minor is not positive definite
         }
         if (nrhs > 0) {
-            // y [n] | t [TB] | ticket
-            if (!cuda_ok(cudaMalloc((void **)&scratch, ((size_t)n + TB + 1) * sizeof(double)))) break;
-            double *y = scratch, *t = scratch + n;
-            unsigned *ticket = reinterpret_cast<unsigned *>(scratch + n + TB);
+            // y [n] | part [TB][npart] | ticket
+            const int npart = (n + TC - 1) / TC;
+            if (!cuda_ok(cudaMalloc((void **)&scratch, ((size_t)n + (size_t)TB * npart + 1) * sizeof(double)))) break;
+            double *y = scratch, *part = scratch + n;
+            unsigned *ticket = reinterpret_cast<unsigned *>(scratch + n + (size_t)TB * npart);
             if (!cuda_ok(cudaMemset(ticket, 0, sizeof(double)))) break;
             const int nb = (n + TB - 1) / TB;
             for (int r = 0; r < nrhs; ++r) {
                 double *g = rhs_dev + (size_t)r * n;
                 for (int b = 0; b < nb; ++b) {
                     const int j0 = b * TB, m = n - j0 < TB ? n - j0 : TB, rest = n - j0 - m;
-                    tri_fwd_kernel<<<rest > 0 ? (rest + TT - 1) / TT : 1, TT>>>(V_dev, ld, n, j0, g, y);
+                    tri_fwd_kernel<<<rest > 0 ? (rest + TF - 1) / TF : 1, TF>>>(V_dev, ld, n, j0, g, y);
                 }
                 for (int b = nb - 1; b >= 0; --b) {
                     const int j0 = b * TB, m = n - j0 < TB ? n - j0 : TB;
-                    tri_bwd_kernel<<<m, TT>>>(V_dev, ld, n, j0, y, g, t, ticket);
+                    const int rest = n - j0 - m, chunks = rest > 0 ? (rest + TC - 1) / TC : 1;
+                    tri_bwd_kernel<<<dim3(m, chunks), TT>>>(V_dev, ld, n, j0, y, g, part, npart, ticket);
                 }
             }
             lx::state_count_launches(2 * nb * nrhs);
