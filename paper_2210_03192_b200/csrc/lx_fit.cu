@@ -36,7 +36,8 @@ struct Solver {
     decltype(&cusolverDnDestroyParams) destroy_params = nullptr;
     decltype(&cusolverDnXpotrf_bufferSize) potrf_size = nullptr;
     decltype(&cusolverDnXpotrf) potrf = nullptr;
-    cusolverDnHandle_t handle = nullptr;      // made once, kept for the life of the process
+    cusolverDnHandle_t handle = nullptr;      // made once per device, kept for the life of the process
+    int handle_dev = -1;
 
     template <class F>
     bool sym(F &f, const char *name) {
@@ -54,8 +55,22 @@ struct Solver {
         ok = sym(create, "cusolverDnCreate") && sym(destroy, "cusolverDnDestroy") &&
              sym(create_params, "cusolverDnCreateParams") && sym(destroy_params, "cusolverDnDestroyParams") &&
              sym(potrf_size, "cusolverDnXpotrf_bufferSize") && sym(potrf, "cusolverDnXpotrf");
-        if (ok && create(&handle) != CUSOLVER_STATUS_SUCCESS) ok = false;
         return ok;
+    }
+    // the handle belongs to the device that was current when it was made (lx_init may have moved the library since)
+    bool ensure() {
+        if (!load()) return false;
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) return false;
+        if (handle && handle_dev != cur) {
+            destroy(handle);
+            handle = nullptr;
+        }
+        if (!handle) {
+            if (create(&handle) != CUSOLVER_STATUS_SUCCESS) { handle = nullptr; return false; }
+            handle_dev = cur;
+        }
+        return true;
     }
 };
 
@@ -226,7 +241,7 @@ extern "C" int lx_fit_solve(double *V_dev, long long ld, int n, double *rhs_dev,
     };
     do {
         if (!factored) {
-            if (!g_solver.load()) { rc = LX_EUNSUPPORTED; break; }
+            if (!g_solver.ensure()) { rc = LX_EUNSUPPORTED; break; }
             cusolverDnParams_t prm = nullptr;
             bool ok = g_solver.create_params(&prm) == CUSOLVER_STATUS_SUCCESS;
             // V is symmetric: its row-major image is its column-major image
