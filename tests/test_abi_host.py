@@ -38,8 +38,10 @@ def test_not_initialised_and_strerror(lx):
     assert lx._lib.lx_boys(None, 1, 3, None, None) == lx.LX_ENOTINIT
     h = C.c_void_p()
     assert lx._lib.lx_schedule_create(None, None, None, None, None, 0, C.c_double(0.0), C.byref(h)) == lx.LX_ENOTINIT
-    for code in (0, -1, -2, -3, -5):
-        assert len(lx.lx_strerror(code)) > 0
+    assert lx._lib.lx_metric_2c(None, None, 0) == lx.LX_ENOTINIT
+    assert lx._lib.lx_fit_solve(None, 0, 0, None, 0, 0) == lx.LX_ENOTINIT
+    for code in (0, -1, -2, -3, -5, -6, -7):
+        assert len(lx.lx_strerror(code)) > 0 and lx.lx_strerror(code) != "unknown status"
     assert lx.lx_strerror(-99) == "unknown status"
     assert "sm_100a" in lx.lx_version()
 
